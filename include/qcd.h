@@ -1,0 +1,204 @@
+/*
+ * qcd.h -- C ABI of libqcd_b200.so: Wilson / Wilson-clover Dslash, fused BLAS-1,
+ * CG on M^dag M, reliable-update mixed CG and a Chebyshev driver, as hand-written
+ * sm_100a CUDA kernels.
+ *
+ * Source of the operations.  The paper (arXiv 2001.05706, /root/reference/PAPER.md)
+ * prints no equation; it names the hot path "the D-slash" (Table 2
+ * caption, sec. 4), run in single precision with SU(3) links
+ * "suppressed to 12 real numbers to save the memory bandwidth",
+ * vector operations / reductions as separate kernels (sec. 3) and the
+ * mixed-precision Krylov solvers of its ref. [1].  The formula is the
+ * one in BASELINE.json north_star,
+ *   D psi(x) = psi(x) - kappa sum_mu [ (1-gamma_mu) U_mu(x) psi(x+mu)
+ *                                    + (1+gamma_mu) U_mu(x-mu)^dag psi(x-mu) ],
+ * with the readings listed in DESIGN.md ("Readings", S1..S23 / O1..O8).
+ *
+ * Conventions
+ *  - Every field pointer is a DEVICE pointer owned by the caller, 16-byte aligned.
+ *    The library never allocates field-sized memory; handles are small host structs.
+ *    (qcd_*_host entry points take HOST pointers and say so.)
+ *  - dims = {X,Y,Z,T}, all even and >= 2.  precision = bytes per real: 4 or 8.
+ *  - Boundary (user) layouts, real type = precision:
+ *      gauge  [t][z][y][x][mu=0..3 (x,y,z,t)][row][col][re,im]
+ *      spinor [t][z][y][x][spin 0..3][colour 0..2][re,im]
+ *  - Internal spinor layout (what qcd_hop / qcd_dslash / qcd_cg_solve take):
+ *      full field = even-parity block then odd-parity block; one parity block =
+ *      [chunk][cb], chunk = one 128-bit word (fp32: 2 complex, 6 chunks; fp64: 1
+ *      complex, 12 chunks), complex index = spin*3+colour, cb = checkerboard index
+ *      (lexicographic site index >> 1), parity = (x+y+z+t)&1.
+ *  - All work is enqueued on the stream given to qcd_init.  Calls that return host
+ *    scalars (reductions, solvers) synchronise that stream; the others do not.
+ *  - Return: 0 = QCD_OK; < 0 error; > 0 soft status.  No exceptions, no aborts, no
+ *    printing.  qcd_last_error() returns text for the last error of this thread.
+ *  - There is no CPU fallback anywhere: without a CUDA device every compute call
+ *    returns QCD_ECUDA.
+ */
+#ifndef QCD_B200_H
+#define QCD_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    QCD_OK = 0,
+    QCD_NOCONV = 1,      /* maxiter reached; x still holds the last iterate          */
+    QCD_EINVAL = -1,     /* bad argument (null / misaligned / aliased / odd dims ...) */
+    QCD_EALLOC = -2,     /* small host or device scratch allocation failed           */
+    QCD_ECUDA = -3,      /* CUDA runtime error (text in qcd_last_error)              */
+    QCD_EBREAKDOWN = -4  /* CG breakdown: <p,Np> <= 0 or NaN                          */
+};
+
+enum { QCD_DAGGER = 1 };                       /* flags for qcd_dslash_ex */
+enum { QCD_PARITY_EVEN = 0, QCD_PARITY_ODD = 1, QCD_PARITY_FULL = 2 };
+
+typedef struct qcd_ctx qcd_ctx;
+typedef struct qcd_gauge qcd_gauge;
+typedef struct qcd_clover qcd_clover;
+
+typedef struct {
+    int iters;             /* number of (low-precision) N = M^dag M applies          */
+    int reliable_updates;  /* mixed CG only                                          */
+    int converged;         /* 1 if |r| <= tol |b| was reached                        */
+    int breakdown;
+    double r_iter;         /* iterated (mixed: last fp64-recomputed) residual / |b|  */
+    double r_true;         /* |b - N x| / |b| recomputed from scratch                */
+    double seconds;        /* device time of the solve loop (CUDA events)            */
+    double flops;          /* nominal: 1320/site hop, +504 clover; BLAS uncounted    */
+    double bytes;          /* compulsory bytes moved by hop + BLAS kernels           */
+} qcd_stats;
+
+const char* qcd_last_error(void);
+int qcd_version(void);
+
+/* device: CUDA ordinal.  cuda_stream: a cudaStream_t (NULL = default stream). */
+int qcd_init(int device, void* cuda_stream, qcd_ctx** ctx);
+int qcd_finalize(qcd_ctx* ctx);
+
+/* ---- gauge field (PAPER.md:143 12-real storage) -----------------
+ * qcd_gauge_load reorders `links` (DEVICE, boundary layout, real = precision_in)
+ * into the checkerboarded SoA layout inside `storage` (DEVICE, caller-owned,
+ * qcd_gauge_bytes(dims, precision, reconstruct) bytes), converting precision if
+ * precision_in != precision.  reconstruct = 18 keeps all 9 complex; 12 keeps rows
+ * 0,1 and the kernels rebuild row 2 = conj(row0 x row1).  t_boundary = -1
+ * antiperiodic / +1 periodic in t: it is recorded in the handle and applied to the
+ * spinor hop, never folded into the stored links (reading S4).
+ * The handle keeps pointers into `storage`; qcd_gauge_free frees only the handle. */
+size_t qcd_gauge_bytes(const int dims[4], int precision, int reconstruct);
+int qcd_gauge_load(qcd_ctx* ctx, qcd_gauge** g, const void* links, int precision_in,
+                   void* storage, const int dims[4], int precision, int reconstruct,
+                   int t_boundary);
+int qcd_gauge_free(qcd_gauge* g);
+
+/* ---- clover term (readings O3, S9, S10) ----------------------
+ * Builds, from the links of `g`, Fhat_munu = (Q - Q^dag)/8 over the 4 plaquette
+ * leaves, A(x) = 1 + kappa*csw*sum_{mu<nu} i sigma_munu (x) Fhat_munu(x) as two
+ * Hermitian 6x6 chiral blocks (2 x (6 real diag + 15 complex) = 72 reals/site) and
+ * A^-1; arithmetic in fp64, stored in `precision`.  storage: DEVICE,
+ * qcd_clover_bytes(dims, precision) bytes (A then A^-1). */
+size_t qcd_clover_bytes(const int dims[4], int precision);
+int qcd_clover_build(qcd_ctx* ctx, qcd_clover** c, const qcd_gauge* g, void* storage,
+                     double kappa, double csw, int precision);
+int qcd_clover_free(qcd_clover* c);
+/* Debug / parity: expand A (which=0) or A^-1 (which=1) to boundary-order dense
+ * [t][z][y][x][12][12][re,im] fp64 (DEVICE, V*288 doubles). */
+int qcd_clover_unpack(qcd_ctx* ctx, void* dense, const qcd_clover* c, int which);
+
+/* ---- spinor layout conversion (boundary <-> internal, both DEVICE) ---------------- */
+size_t qcd_spinor_bytes(const int dims[4], int precision);   /* full lattice */
+int qcd_spinor_pack(qcd_ctx* ctx, void* internal, const void* boundary, const int dims[4],
+                    int precision);
+int qcd_spinor_unpack(qcd_ctx* ctx, void* boundary, const void* internal, const int dims[4],
+                      int precision);
+/* precision conversion of an internal-layout array of n reals (n multiple of 4) */
+int qcd_convert(qcd_ctx* ctx, void* dst, int precision_dst, const void* src, int precision_src,
+                size_t nreal);
+
+/* ---- the stencil (north_star formula) --------------------------
+ * qcd_hop: raw single-parity hopping term, the kernel the 1320 flop/site figure is
+ * for:  out_p = H_{p,1-p} in_{1-p}   (dagger: H^dag, projector signs swapped).
+ * `out`, `in`: ONE-parity internal blocks (Vh*24 reals), must not alias.
+ * qcd_hop_xpay: out_p = a * z_p + b * H_{p,1-p} in_{1-p}  (z may alias out). */
+int qcd_hop(void* out, const void* in, const qcd_gauge* g, int out_parity, int dagger,
+            const int dims[4], int precision);
+int qcd_hop_xpay(void* out, const void* in, const void* z, double a, double b,
+                 const qcd_gauge* g, int out_parity, int dagger);
+
+/* qcd_dslash (north_star signature):
+ *   parity = 2: full lattice, out = (A - kappa H) in; in/out = full internal fields
+ *               (A = 1 when clover == NULL);
+ *   parity = 0|1: even-odd preconditioned operator on that parity (reading O5),
+ *               out_p = A_pp in_p - kappa^2 H_{p,pb} A^-1_{pb,pb} H_{pb,p} in_p,
+ *               in/out = one-parity blocks.  Needs a Vh*24-real temporary: use
+ *               qcd_dslash_ex with tmp, or qcd_dslash allocates nothing and returns
+ *               QCD_EINVAL if the ctx has no workspace set (qcd_set_workspace).
+ * kappa/csw must equal the values the clover handle was built with (S10).
+ * dims/precision must match the gauge handle.  in and out must not alias. */
+int qcd_dslash(void* out, const void* in, const qcd_gauge* gauge, const qcd_clover* clover,
+               double kappa, double csw, int parity, const int dims[4], int precision);
+int qcd_dslash_ex(void* out, const void* in, const qcd_gauge* gauge, const qcd_clover* clover,
+                  double kappa, double csw, int parity, int flags, void* tmp);
+
+/* ---- workspace ----------------------------------------------------------------------
+ * Caller-provided DEVICE scratch used by qcd_dslash (parity 0|1), the solvers and the
+ * Chebyshev driver.  qcd_workspace_bytes gives the size that covers every call for
+ * this lattice (precision = the highest precision used). */
+size_t qcd_workspace_bytes(const int dims[4], int precision);
+int qcd_set_workspace(qcd_ctx* ctx, void* ws, size_t bytes);
+
+/* ---- fused BLAS-1 ("vector operations", reductions) --
+ * Arrays of `nreal` reals (multiple of 4) in `precision`.  Reductions multiply and
+ * accumulate in fp64 (warp shuffle -> block -> last-block final pass, fixed order,
+ * deterministic) and return the scalar to the HOST pointer (synchronises).        */
+int qcd_axpy(qcd_ctx*, double a, const void* x, void* y, size_t nreal, int precision);   /* y += a x   */
+int qcd_xpay(qcd_ctx*, const void* x, double a, void* y, size_t nreal, int precision);   /* y = x + a y */
+int qcd_axpby(qcd_ctx*, double a, const void* x, double b, void* y, size_t nreal, int precision); /* y = a x + b y */
+int qcd_norm2(qcd_ctx*, const void* x, size_t nreal, int precision, double* result);
+int qcd_redot(qcd_ctx*, const void* x, const void* y, size_t nreal, int precision, double* result); /* Re<x,y> */
+/* x += a p; r -= a q; *result = |r|^2  (the CG update, one pass) */
+int qcd_cg_update(qcd_ctx*, double a, const void* p, const void* q, void* x, void* r,
+                  size_t nreal, int precision, double* result);
+
+/* ---- solvers (readings O6, O7, S13, S15) ----------------------
+ * qcd_set_operator selects M for the solvers of this ctx:
+ *   parity 2: M = A - kappa H on the full lattice; 0|1: even-odd Schur operator.
+ *   g_lo/c_lo != NULL selects the reliable-update mixed solver (fp32 inner iteration
+ *   with g_lo/c_lo, fp64 true residual with g_hi/c_hi, threshold delta).
+ * qcd_cg_solve solves (M^dag M) x = b, x0 = 0 (input x ignored), x and b in the
+ * precision of g_hi, internal layout (full field for parity 2, one block else).
+ * Stops when the iterated residual |r| <= tol |b| (tested after the update).
+ * Returns QCD_OK, QCD_NOCONV, QCD_EBREAKDOWN or an error.  Uses the ctx that last
+ * called qcd_set_operator (qcd_cg_solve_ex names it). */
+int qcd_set_operator(qcd_ctx* ctx, const qcd_gauge* g_hi, const qcd_gauge* g_lo,
+                     const qcd_clover* c_hi, const qcd_clover* c_lo, double kappa, double csw,
+                     int parity, double delta);
+int qcd_cg_solve(void* x, const void* b, double tol, int maxiter);
+int qcd_cg_solve_ex(qcd_ctx* ctx, void* x, const void* b, double tol, int maxiter,
+                    qcd_stats* stats);
+/* out = M in (flags & QCD_DAGGER: M^dag in) for the operator of qcd_set_operator, in
+ * the high precision. */
+int qcd_apply_operator(qcd_ctx* ctx, void* out, const void* in, int flags);
+
+/* ---- Chebyshev driver (reading O8/S16) -----------
+ * y = sum_{k=0}^{degree} coeff[k] T_k(H_W/scale) v,  H_W = gamma5 (1 - kappa H), full
+ * lattice, forward three-term recurrence.  v, y: full internal fields in the gauge's
+ * precision; coeff: HOST array of degree+1 doubles.  Uses the ctx workspace. */
+int qcd_cheb_apply(qcd_ctx* ctx, void* y, const void* v, const qcd_gauge* g, double kappa,
+                   const double* coeff, int degree, double scale);
+
+/* ---- host-buffer convenience (end-to-end path: copies inside the call) -------------
+ * out_host = H_{p,1-p} in_host for one-parity blocks held in HOST memory, internal
+ * layout: copies in -> device scratch (ctx workspace), runs qcd_hop, copies out. */
+int qcd_hop_host(qcd_ctx* ctx, void* out_host, const void* in_host, const qcd_gauge* g,
+                 int out_parity, int dagger);
+
+/* number of kernels this library has launched on this ctx since qcd_init */
+long long qcd_launch_count(const qcd_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QCD_B200_H */
