@@ -1,0 +1,408 @@
+/*
+ * api.cu -- the C ABI of include/qcd.h: handles, argument checking, layout and operator
+ * entry points.  Solvers and the Chebyshev driver are in solver.cu.
+ */
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "qcd_internal.h"
+
+static thread_local char g_err[512] = "";
+
+int qcd_set_error(int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+static int make_geom(const int dims[4], Geom* g)
+{
+    if (!dims) return qcd_set_error(QCD_EINVAL, "dims is NULL");
+    for (int i = 0; i < 4; i++)
+        if (dims[i] < 2 || (dims[i] & 1)) return qcd_set_error(QCD_EINVAL, "dims[%d]=%d must be even and >= 2", i, dims[i]);
+    g->X = dims[0]; g->Y = dims[1]; g->Z = dims[2]; g->T = dims[3];
+    g->X2 = g->X / 2;
+    g->V = (long long)g->X * g->Y * g->Z * g->T;
+    if (g->V / 2 > 0x3fffffffLL) return qcd_set_error(QCD_EINVAL, "lattice too large for 32-bit site indices");
+    g->Vh = (int)(g->V / 2);
+    return QCD_OK;
+}
+static bool same_dims(const Geom& g, const int dims[4])
+{
+    return dims && g.X == dims[0] && g.Y == dims[1] && g.Z == dims[2] && g.T == dims[3];
+}
+static bool aligned16(const void* p) { return p && (((uintptr_t)p) & 15u) == 0; }
+static bool overlap(const void* a, const void* b, size_t bytes)
+{
+    const uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
+    return x < y + bytes && y < x + bytes;
+}
+
+extern "C" {
+
+const char* qcd_last_error(void) { return g_err; }
+int qcd_version(void) { return 100; }
+
+int qcd_init(int device, void* cuda_stream, qcd_ctx** out)
+{
+    if (!out) return qcd_set_error(QCD_EINVAL, "ctx is NULL");
+    *out = nullptr;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0)
+        return qcd_set_error(QCD_ECUDA, "no CUDA device (%s); this library has no CPU fallback", cudaGetErrorString(e));
+    if (device < 0 || device >= ndev) return qcd_set_error(QCD_EINVAL, "device %d out of range", device);
+    QCD_CHECK_CUDA(cudaSetDevice(device));
+    qcd_ctx* c = (qcd_ctx*)calloc(1, sizeof(qcd_ctx));
+    if (!c) return qcd_set_error(QCD_EALLOC, "ctx alloc");
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    cudaDeviceProp prop;
+    QCD_CHECK_CUDA(cudaGetDeviceProperties(&prop, device));
+    c->num_sms = prop.multiProcessorCount;
+    c->max_blocks = c->num_sms * 8; /* 8 resident 256-thread blocks per SM */
+    e = cudaMalloc(&c->d_partial, sizeof(double) * (size_t)c->max_blocks);
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_ticket, sizeof(unsigned int) * 64);
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_scalar, sizeof(double) * SC_COUNT);
+    if (e == cudaSuccess) e = cudaMallocHost(&c->h_scalar, sizeof(double) * SC_COUNT);
+    if (e == cudaSuccess) e = cudaMemset(c->d_ticket, 0, sizeof(unsigned int) * 64);
+    if (e == cudaSuccess) e = cudaMemset(c->d_scalar, 0, sizeof(double) * SC_COUNT);
+    if (e != cudaSuccess) {
+        qcd_finalize(c);
+        return qcd_set_error(QCD_EALLOC, "scratch allocation: %s", cudaGetErrorString(e));
+    }
+    *out = c;
+    return QCD_OK;
+}
+
+int qcd_finalize(qcd_ctx* c)
+{
+    if (!c) return QCD_OK;
+    if (c->d_partial) cudaFree(c->d_partial);
+    if (c->d_ticket) cudaFree(c->d_ticket);
+    if (c->d_scalar) cudaFree(c->d_scalar);
+    if (c->h_scalar) cudaFreeHost(c->h_scalar);
+    free(c);
+    return QCD_OK;
+}
+
+long long qcd_launch_count(const qcd_ctx* c) { return c ? c->launches : 0; }
+
+/* ---- gauge ------------------------------------------------------------------------ */
+size_t qcd_gauge_bytes(const int dims[4], int precision, int reconstruct)
+{
+    Geom g;
+    if (make_geom(dims, &g) != QCD_OK) return 0;
+    if ((precision != 4 && precision != 8) || (reconstruct != 12 && reconstruct != 18)) return 0;
+    return 8 * gauge_block_bytes(g, precision, reconstruct);
+}
+
+int qcd_gauge_load(qcd_ctx* ctx, qcd_gauge** out, const void* links, int precision_in, void* storage, const int dims[4],
+                   int precision, int reconstruct, int t_boundary)
+{
+    QCD_REQUIRE(ctx && out, "gauge_load: NULL ctx/handle");
+    *out = nullptr;
+    Geom g;
+    int rc = make_geom(dims, &g);
+    if (rc) return rc;
+    QCD_REQUIRE(precision == 4 || precision == 8, "gauge_load: precision must be 4|8");
+    QCD_REQUIRE(precision_in == 4 || precision_in == 8, "gauge_load: precision_in must be 4|8");
+    QCD_REQUIRE(reconstruct == 12 || reconstruct == 18, "gauge_load: reconstruct must be 12|18");
+    QCD_REQUIRE(t_boundary == 1 || t_boundary == -1, "gauge_load: t_boundary must be +1|-1");
+    QCD_REQUIRE(aligned16(links) && aligned16(storage), "gauge_load: pointers must be non-NULL and 16-byte aligned");
+    qcd_gauge* h = (qcd_gauge*)calloc(1, sizeof(qcd_gauge));
+    if (!h) return qcd_set_error(QCD_EALLOC, "gauge handle");
+    h->ctx = ctx; h->geo = g; h->precision = precision; h->reconstruct = reconstruct; h->tb = t_boundary;
+    h->data = storage;
+    h->block_bytes = gauge_block_bytes(g, precision, reconstruct);
+    rc = layout_gauge_load(ctx, h, links, precision_in);
+    if (rc) { free(h); return rc; }
+    *out = h;
+    return QCD_OK;
+}
+int qcd_gauge_free(qcd_gauge* g) { free(g); return QCD_OK; }
+
+/* ---- clover ------------------------------------------------------------------------- */
+size_t qcd_clover_bytes(const int dims[4], int precision)
+{
+    Geom g;
+    if (make_geom(dims, &g) != QCD_OK) return 0;
+    if (precision != 4 && precision != 8) return 0;
+    return (size_t)4 * g.Vh * 72 * precision; /* A[2 parities] + Ainv[2 parities] */
+}
+
+int qcd_clover_build(qcd_ctx* ctx, qcd_clover** out, const qcd_gauge* g, void* storage, double kappa, double csw, int precision)
+{
+    QCD_REQUIRE(ctx && out && g, "clover_build: NULL argument");
+    *out = nullptr;
+    QCD_REQUIRE(precision == 4 || precision == 8, "clover_build: precision must be 4|8");
+    QCD_REQUIRE(aligned16(storage), "clover_build: storage must be non-NULL and 16-byte aligned");
+    qcd_clover* c = (qcd_clover*)calloc(1, sizeof(qcd_clover));
+    if (!c) return qcd_set_error(QCD_EALLOC, "clover handle");
+    c->ctx = ctx; c->geo = g->geo; c->precision = precision; c->kappa = kappa; c->csw = csw;
+    c->data = storage;
+    c->block_bytes = (size_t)g->geo.Vh * 72 * precision;
+    int rc = clover_build(ctx, g, c);
+    if (rc) { free(c); return rc; }
+    *out = c;
+    return QCD_OK;
+}
+int qcd_clover_free(qcd_clover* c) { free(c); return QCD_OK; }
+
+int qcd_clover_unpack(qcd_ctx* ctx, void* dense, const qcd_clover* c, int which)
+{
+    QCD_REQUIRE(ctx && c && aligned16(dense), "clover_unpack: bad argument");
+    QCD_REQUIRE(which == 0 || which == 1, "clover_unpack: which must be 0|1");
+    return clover_unpack(ctx, dense, c, which);
+}
+
+/* ---- spinor layout ------------------------------------------------------------------ */
+size_t qcd_spinor_bytes(const int dims[4], int precision)
+{
+    Geom g;
+    if (make_geom(dims, &g) != QCD_OK) return 0;
+    if (precision != 4 && precision != 8) return 0;
+    return (size_t)g.V * 24 * precision;
+}
+
+static int pack_common(qcd_ctx* ctx, void* internal, const void* boundary, const int dims[4], int precision, int unpack)
+{
+    QCD_REQUIRE(ctx, "spinor pack: NULL ctx");
+    Geom g;
+    int rc = make_geom(dims, &g);
+    if (rc) return rc;
+    QCD_REQUIRE(precision == 4 || precision == 8, "spinor pack: precision must be 4|8");
+    QCD_REQUIRE(aligned16(internal) && aligned16(boundary), "spinor pack: pointers must be non-NULL, 16-byte aligned");
+    QCD_REQUIRE(!overlap(internal, boundary, (size_t)g.V * 24 * precision), "spinor pack: buffers alias");
+    return layout_spinor_pack(ctx, internal, boundary, g, precision, unpack);
+}
+int qcd_spinor_pack(qcd_ctx* ctx, void* internal, const void* boundary, const int dims[4], int precision)
+{
+    return pack_common(ctx, internal, boundary, dims, precision, 0);
+}
+int qcd_spinor_unpack(qcd_ctx* ctx, void* boundary, const void* internal, const int dims[4], int precision)
+{
+    return pack_common(ctx, const_cast<void*>(internal), boundary, dims, precision, 1);
+}
+
+int qcd_convert(qcd_ctx* ctx, void* dst, int pd, const void* src, int ps, size_t nreal)
+{
+    QCD_REQUIRE(ctx && aligned16(dst) && aligned16(src), "convert: bad pointer");
+    QCD_REQUIRE((pd == 4 || pd == 8) && (ps == 4 || ps == 8), "convert: precision must be 4|8");
+    return blas_convert(ctx, dst, pd, src, ps, nreal);
+}
+
+/* ---- workspace ------------------------------------------------------------------------ */
+size_t qcd_workspace_bytes(const int dims[4], int precision)
+{
+    Geom g;
+    if (make_geom(dims, &g) != QCD_OK) return 0;
+    if (precision != 4 && precision != 8) return 0;
+    /* pure CG: r,p,q,t,tmp (5); mixed CG: 4 fp64 + 6 fp32 = 7 fp64-equivalents; Chebyshev: 2 */
+    return (size_t)8 * g.V * 24 * precision;
+}
+int qcd_set_workspace(qcd_ctx* ctx, void* ws, size_t bytes)
+{
+    QCD_REQUIRE(ctx, "set_workspace: NULL ctx");
+    QCD_REQUIRE(ws == nullptr || aligned16(ws), "set_workspace: misaligned");
+    ctx->ws = ws;
+    ctx->ws_bytes = ws ? bytes : 0;
+    return QCD_OK;
+}
+
+/* ---- the stencil ------------------------------------------------------------------------ */
+int qcd_hop_xpay(void* out, const void* in, const void* z, double a, double b, const qcd_gauge* g, int out_parity, int dagger)
+{
+    QCD_REQUIRE(g && g->ctx, "hop: NULL gauge");
+    const size_t bytes = (size_t)g->geo.Vh * 24 * g->precision;
+    QCD_REQUIRE(aligned16(out) && aligned16(in), "hop: pointers must be non-NULL, 16-byte aligned");
+    QCD_REQUIRE(!overlap(out, in, bytes), "hop: in and out alias");
+    QCD_REQUIRE(out_parity == 0 || out_parity == 1, "hop: out_parity must be 0|1");
+    HopLaunch L;
+    memset(&L, 0, sizeof(L));
+    L.out = out; L.in = in; L.out_parity = out_parity; L.dagger = dagger ? 1 : 0;
+    if (z) {
+        QCD_REQUIRE(aligned16(z) && !overlap(z, in, bytes), "hop_xpay: z misaligned or aliases in");
+        L.mode = HOP_XPAY; L.z = z; L.a = a; L.b = b;
+    } else {
+        L.mode = HOP_PLAIN;
+    }
+    return hop_launch(g->ctx, g, L);
+}
+
+int qcd_hop(void* out, const void* in, const qcd_gauge* g, int out_parity, int dagger, const int dims[4], int precision)
+{
+    QCD_REQUIRE(g, "hop: NULL gauge");
+    QCD_REQUIRE(same_dims(g->geo, dims) && precision == g->precision, "hop: dims/precision do not match the gauge handle");
+    return qcd_hop_xpay(out, in, nullptr, 0.0, 0.0, g, out_parity, dagger);
+}
+
+} /* extern "C" */
+
+/* out_p = A_pp in_p - kappa H_{p,pb} in_pb for both parities (full lattice) */
+static int apply_full(qcd_ctx* ctx, void* out, const void* in, const qcd_gauge* g, const qcd_clover* c, double kappa, int dagger)
+{
+    const size_t blk = (size_t)g->geo.Vh * 24 * g->precision;
+    for (int p = 0; p < 2; p++) {
+        HopLaunch L;
+        memset(&L, 0, sizeof(L));
+        L.out = (char*)out + p * blk;
+        L.in = (const char*)in + (1 - p) * blk;
+        L.z = (const char*)in + p * blk;
+        L.a = 1.0; L.b = -kappa;
+        L.out_parity = p; L.dagger = dagger;
+        if (c) { L.mode = HOP_CLOVER_Z; L.clover = (const char*)c->data + p * c->block_bytes; }
+        else L.mode = HOP_XPAY;
+        int rc = hop_launch(ctx, g, L);
+        if (rc) return rc;
+    }
+    return QCD_OK;
+}
+
+/* even-odd Schur operator (reading O5):
+ *   tmp_pb = Ainv_pb H_{pb,p} in_p ;  out_p = A_pp in_p - kappa^2 H_{p,pb} tmp_pb */
+static int apply_eo(qcd_ctx* ctx, void* out, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c, double kappa, int p,
+                    int dagger)
+{
+    HopLaunch L;
+    memset(&L, 0, sizeof(L));
+    L.out = tmp; L.in = in; L.out_parity = 1 - p; L.dagger = dagger;
+    if (c) { L.mode = HOP_CLOVER_OUT; L.clover = (const char*)c->data + (2 + (1 - p)) * c->block_bytes; }
+    else L.mode = HOP_PLAIN;
+    int rc = hop_launch(ctx, g, L);
+    if (rc) return rc;
+    memset(&L, 0, sizeof(L));
+    L.out = out; L.in = tmp; L.z = in; L.a = 1.0; L.b = -kappa * kappa; L.out_parity = p; L.dagger = dagger;
+    if (c) { L.mode = HOP_CLOVER_Z; L.clover = (const char*)c->data + p * c->block_bytes; }
+    else L.mode = HOP_XPAY;
+    return hop_launch(ctx, g, L);
+}
+
+int op_apply_M(qcd_ctx* ctx, void* out, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c, double kappa, int parity,
+               int dagger)
+{
+    if (parity == QCD_PARITY_FULL) return apply_full(ctx, out, in, g, c, kappa, dagger);
+    return apply_eo(ctx, out, in, tmp, g, c, kappa, parity, dagger);
+}
+
+extern "C" {
+
+int qcd_dslash_ex(void* out, const void* in, const qcd_gauge* g, const qcd_clover* c, double kappa, double csw, int parity, int flags,
+                  void* tmp)
+{
+    QCD_REQUIRE(g && g->ctx, "dslash: NULL gauge");
+    qcd_ctx* ctx = g->ctx;
+    QCD_REQUIRE(parity == 0 || parity == 1 || parity == 2, "dslash: parity must be 0|1|2");
+    QCD_REQUIRE(aligned16(out) && aligned16(in), "dslash: pointers must be non-NULL, 16-byte aligned");
+    const size_t blk = (size_t)g->geo.Vh * 24 * g->precision;
+    const size_t bytes = parity == 2 ? 2 * blk : blk;
+    QCD_REQUIRE(!overlap(out, in, bytes), "dslash: in and out alias");
+    if (c) {
+        QCD_REQUIRE(c->precision == g->precision && c->geo.V == g->geo.V, "dslash: clover does not match gauge");
+        QCD_REQUIRE(c->kappa == kappa && c->csw == csw, "dslash: kappa/csw differ from the values the clover was built with");
+    }
+    if (parity != 2) {
+        if (!tmp) {
+            QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= blk, "dslash: parity 0|1 needs a temporary (qcd_set_workspace or tmp)");
+            tmp = ctx->ws;
+        }
+        QCD_REQUIRE(aligned16(tmp) && !overlap(tmp, in, blk) && !overlap(tmp, out, blk), "dslash: tmp misaligned or aliased");
+    }
+    return op_apply_M(ctx, out, in, tmp, g, c, kappa, parity, (flags & QCD_DAGGER) ? 1 : 0);
+}
+
+int qcd_dslash(void* out, const void* in, const qcd_gauge* g, const qcd_clover* c, double kappa, double csw, int parity,
+               const int dims[4], int precision)
+{
+    QCD_REQUIRE(g, "dslash: NULL gauge");
+    QCD_REQUIRE(same_dims(g->geo, dims) && precision == g->precision, "dslash: dims/precision do not match the gauge handle");
+    return qcd_dslash_ex(out, in, g, c, kappa, csw, parity, 0, nullptr);
+}
+
+/* ---- BLAS ------------------------------------------------------------------------------ */
+static int blas_args(qcd_ctx* ctx, const void* x, const void* y, size_t nreal, int precision)
+{
+    QCD_REQUIRE(ctx, "blas: NULL ctx");
+    QCD_REQUIRE(precision == 4 || precision == 8, "blas: precision must be 4|8");
+    QCD_REQUIRE(nreal % 4 == 0, "blas: nreal must be a multiple of 4");
+    QCD_REQUIRE(aligned16(x) && aligned16(y), "blas: pointers must be non-NULL, 16-byte aligned");
+    return QCD_OK;
+}
+static int fetch_scalar(qcd_ctx* ctx, int slot, double* result)
+{
+    QCD_CHECK_CUDA(cudaMemcpyAsync(ctx->h_scalar + slot, ctx->d_scalar + slot, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    QCD_CHECK_CUDA(cudaStreamSynchronize(ctx->stream));
+    *result = ctx->h_scalar[slot];
+    return QCD_OK;
+}
+
+int qcd_axpy(qcd_ctx* ctx, double a, const void* x, void* y, size_t nreal, int precision)
+{
+    int rc = blas_args(ctx, x, y, nreal, precision);
+    if (rc) return rc;
+    return blas_axpby(ctx, host_scalar(a), x, host_scalar(1.0), y, nreal, precision);
+}
+int qcd_xpay(qcd_ctx* ctx, const void* x, double a, void* y, size_t nreal, int precision)
+{
+    int rc = blas_args(ctx, x, y, nreal, precision);
+    if (rc) return rc;
+    return blas_axpby(ctx, host_scalar(1.0), x, host_scalar(a), y, nreal, precision);
+}
+int qcd_axpby(qcd_ctx* ctx, double a, const void* x, double b, void* y, size_t nreal, int precision)
+{
+    int rc = blas_args(ctx, x, y, nreal, precision);
+    if (rc) return rc;
+    return blas_axpby(ctx, host_scalar(a), x, host_scalar(b), y, nreal, precision);
+}
+int qcd_norm2(qcd_ctx* ctx, const void* x, size_t nreal, int precision, double* result)
+{
+    int rc = blas_args(ctx, x, x, nreal, precision);
+    if (rc) return rc;
+    QCD_REQUIRE(result, "norm2: NULL result");
+    rc = blas_norm2(ctx, x, nreal, precision, ctx->d_scalar + SC_TMP);
+    if (rc) return rc;
+    return fetch_scalar(ctx, SC_TMP, result);
+}
+int qcd_redot(qcd_ctx* ctx, const void* x, const void* y, size_t nreal, int precision, double* result)
+{
+    int rc = blas_args(ctx, x, y, nreal, precision);
+    if (rc) return rc;
+    QCD_REQUIRE(result, "redot: NULL result");
+    rc = blas_redot(ctx, x, y, nreal, precision, ctx->d_scalar + SC_TMP);
+    if (rc) return rc;
+    return fetch_scalar(ctx, SC_TMP, result);
+}
+int qcd_cg_update(qcd_ctx* ctx, double a, const void* p, const void* q, void* x, void* r, size_t nreal, int precision, double* result)
+{
+    int rc = blas_args(ctx, p, q, nreal, precision);
+    if (rc) return rc;
+    rc = blas_args(ctx, x, r, nreal, precision);
+    if (rc) return rc;
+    QCD_REQUIRE(result, "cg_update: NULL result");
+    rc = blas_cg_update(ctx, host_scalar(a), p, q, x, r, nreal, precision, ctx->d_scalar + SC_TMP, nullptr, nullptr);
+    if (rc) return rc;
+    return fetch_scalar(ctx, SC_TMP, result);
+}
+
+/* ---- host-buffer end-to-end path ----------------------------------------------------------- */
+int qcd_hop_host(qcd_ctx* ctx, void* out_host, const void* in_host, const qcd_gauge* g, int out_parity, int dagger)
+{
+    QCD_REQUIRE(ctx && g && out_host && in_host, "hop_host: NULL argument");
+    const size_t blk = (size_t)g->geo.Vh * 24 * g->precision;
+    QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= 2 * blk, "hop_host: workspace too small (qcd_set_workspace)");
+    char* d_in = (char*)ctx->ws;
+    char* d_out = d_in + blk;
+    QCD_CHECK_CUDA(cudaMemcpyAsync(d_in, in_host, blk, cudaMemcpyHostToDevice, ctx->stream));
+    int rc = qcd_hop_xpay(d_out, d_in, nullptr, 0.0, 0.0, g, out_parity, dagger);
+    if (rc) return rc;
+    QCD_CHECK_CUDA(cudaMemcpyAsync(out_host, d_out, blk, cudaMemcpyDeviceToHost, ctx->stream));
+    QCD_CHECK_CUDA(cudaStreamSynchronize(ctx->stream));
+    return QCD_OK;
+}
+
+} /* extern "C" */

@@ -1,0 +1,278 @@
+/*
+ * blas.cu -- fused BLAS-1 for the CG ("vector
+ * operations" and reductions as their own kernels).  All streams are 128-bit loads /
+ * stores; every reduction multiplies and accumulates in fp64 and is deterministic:
+ * fixed grid, per-thread strided sum -> warp shuffle tree -> shared-memory tree ->
+ * per-block partial -> the last block to finish (ticket) sums the partials in a fixed
+ * order and writes the scalar (and derived scalars) to device memory.
+ */
+#include "qcd_device.cuh"
+
+namespace {
+
+constexpr int BLAS_THREADS = 256;
+
+__device__ __forceinline__ double eval(const DevScalar& s)
+{
+    return s.num ? s.sign * (*s.num / *s.den) : s.val;
+}
+
+__device__ __forceinline__ double block_sum(double v)
+{
+    __shared__ double sm[BLAS_THREADS / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads();
+    if (l == 0) sm[w] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (w == 0) {
+        r = (l < BLAS_THREADS / 32) ? sm[l] : 0.0;
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
+    }
+    return r; /* valid in thread 0 */
+}
+
+/* Second stage.  Returns true (in thread 0 of the last block) with the total in *tot. */
+__device__ __forceinline__ bool grid_sum(double v, double* partial, unsigned int* ticket, double* tot)
+{
+    __shared__ bool last;
+    const double bs = block_sum(v);
+    if (threadIdx.x == 0) {
+        partial[blockIdx.x] = bs;
+        __threadfence();
+        const unsigned int t = atomicInc(ticket, gridDim.x - 1); /* wraps back to 0 */
+        last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!last) return false;
+    __threadfence();
+    double s = 0.0;
+    for (unsigned int i = threadIdx.x; i < gridDim.x; i += BLAS_THREADS) s += ((volatile double*)partial)[i];
+    const double r = block_sum(s);
+    if (threadIdx.x == 0) *tot = r;
+    return threadIdx.x == 0;
+}
+
+template <typename T> __global__ void __launch_bounds__(BLAS_THREADS) axpby_kernel(DevScalar a, const T* x, DevScalar b, T* y, size_t nvec)
+{
+    typedef typename Vec<T>::type V;
+    const T aa = (T)eval(a), bb = (T)eval(b);
+    const V* xv = reinterpret_cast<const V*>(x);
+    V* yv = reinterpret_cast<V*>(y);
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
+        T xs[Vec<T>::reals], ys[Vec<T>::reals];
+        vec_get(xv[i], xs);
+        vec_get(yv[i], ys);
+#pragma unroll
+        for (int k = 0; k < Vec<T>::reals; k++) ys[k] = aa * xs[k] + bb * ys[k];
+        yv[i] = vec_make(ys);
+    }
+}
+
+template <typename T, int TWO>
+__global__ void __launch_bounds__(BLAS_THREADS) dot_kernel(const T* x, const T* y, size_t nvec, double* partial, unsigned int* ticket, double* out)
+{
+    typedef typename Vec<T>::type V;
+    const V* xv = reinterpret_cast<const V*>(x);
+    const V* yv = reinterpret_cast<const V*>(y);
+    double s = 0.0;
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
+        T xs[Vec<T>::reals], ys[Vec<T>::reals];
+        vec_get(xv[i], xs);
+        if (TWO) vec_get(yv[i], ys);
+#pragma unroll
+        for (int k = 0; k < Vec<T>::reals; k++) s += (double)xs[k] * (double)(TWO ? ys[k] : xs[k]);
+    }
+    double tot;
+    if (grid_sum(s, partial, ticket, &tot)) *out = tot;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(BLAS_THREADS) cg_update_kernel(DevScalar a, const T* p, const T* q, T* x, T* r, size_t nvec, double* partial,
+                                 unsigned int* ticket, double* out, double* beta, const double* rho_old)
+{
+    typedef typename Vec<T>::type V;
+    const T aa = (T)eval(a);
+    const V* pv = reinterpret_cast<const V*>(p);
+    const V* qv = reinterpret_cast<const V*>(q);
+    V* xv = reinterpret_cast<V*>(x);
+    V* rv = reinterpret_cast<V*>(r);
+    double s = 0.0;
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
+        T ps[Vec<T>::reals], qs[Vec<T>::reals], xs[Vec<T>::reals], rs[Vec<T>::reals];
+        vec_get(pv[i], ps);
+        vec_get(qv[i], qs);
+        vec_get(xv[i], xs);
+        vec_get(rv[i], rs);
+#pragma unroll
+        for (int k = 0; k < Vec<T>::reals; k++) {
+            xs[k] += aa * ps[k];
+            rs[k] -= aa * qs[k];
+            s += (double)rs[k] * (double)rs[k];
+        }
+        xv[i] = vec_make(xs);
+        rv[i] = vec_make(rs);
+    }
+    double tot;
+    if (grid_sum(s, partial, ticket, &tot)) {
+        *out = tot;
+        if (beta) *beta = tot / *rho_old;
+    }
+}
+
+/* y_hi += x_lo ; x_lo = 0   (reliable update, reading O7) */
+__global__ void __launch_bounds__(BLAS_THREADS) accumulate_hi_kernel(double* y, float* x, size_t n4)
+{
+    float4* xv = reinterpret_cast<float4*>(x);
+    double2* yv = reinterpret_cast<double2*>(y);
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < n4; i += (size_t)gridDim.x * BLAS_THREADS) {
+        const float4 v = xv[i];
+        double2 a = yv[2 * i], b = yv[2 * i + 1];
+        a.x += (double)v.x; a.y += (double)v.y; b.x += (double)v.z; b.y += (double)v.w;
+        yv[2 * i] = a;
+        yv[2 * i + 1] = b;
+        xv[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
+/* r_hi = b - t ; r_lo = (float) r_hi ; out = |r_hi|^2 */
+__global__ void __launch_bounds__(BLAS_THREADS) residual_hi_kernel(double* rh, float* rl, const double* b, const double* t, size_t n4, double* partial,
+                                   unsigned int* ticket, double* out)
+{
+    double s = 0.0;
+    const double2* bv = reinterpret_cast<const double2*>(b);
+    const double2* tv = reinterpret_cast<const double2*>(t);
+    double2* rv = reinterpret_cast<double2*>(rh);
+    float4* lv = reinterpret_cast<float4*>(rl);
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < n4; i += (size_t)gridDim.x * BLAS_THREADS) {
+        const double2 b0 = bv[2 * i], b1 = bv[2 * i + 1], t0 = tv[2 * i], t1 = tv[2 * i + 1];
+        const double2 r0 = make_double2(b0.x - t0.x, b0.y - t0.y), r1 = make_double2(b1.x - t1.x, b1.y - t1.y);
+        s += r0.x * r0.x + r0.y * r0.y + r1.x * r1.x + r1.y * r1.y;
+        rv[2 * i] = r0;
+        rv[2 * i + 1] = r1;
+        if (rl) lv[i] = make_float4((float)r0.x, (float)r0.y, (float)r1.x, (float)r1.y);
+    }
+    double tot;
+    if (grid_sum(s, partial, ticket, &tot)) *out = tot;
+}
+
+template <typename D, typename S> __global__ void __launch_bounds__(BLAS_THREADS) convert_kernel(D* dst, const S* src, size_t n)
+{
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_THREADS) dst[i] = (D)src[i];
+}
+
+int grid_for(const qcd_ctx* ctx, size_t nvec)
+{
+    size_t b = (nvec + BLAS_THREADS - 1) / BLAS_THREADS;
+    const size_t cap = (size_t)ctx->max_blocks;
+    if (b > cap) b = cap;
+    if (b < 1) b = 1;
+    return (int)b;
+}
+
+int check_launch(qcd_ctx* ctx, const char* what)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+    ctx->launches++;
+    return QCD_OK;
+}
+
+} // namespace
+
+int blas_axpby(qcd_ctx* ctx, DevScalar a, const void* x, DevScalar b, void* y, size_t nreal, int prec)
+{
+    if (prec == 4) {
+        const size_t nv = nreal / 4;
+        axpby_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const float*)x, b, (float*)y, nv);
+    } else {
+        const size_t nv = nreal / 2;
+        axpby_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const double*)x, b, (double*)y, nv);
+    }
+    return check_launch(ctx, "axpby");
+}
+
+int blas_norm2(qcd_ctx* ctx, const void* x, size_t nreal, int prec, double* d_out)
+{
+    if (prec == 4) {
+        const size_t nv = nreal / 4;
+        dot_kernel<float, 0><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const float*)x, (const float*)x, nv, ctx->d_partial, ctx->d_ticket, d_out);
+    } else {
+        const size_t nv = nreal / 2;
+        dot_kernel<double, 0><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const double*)x, (const double*)x, nv, ctx->d_partial, ctx->d_ticket, d_out);
+    }
+    return check_launch(ctx, "norm2");
+}
+
+int blas_redot(qcd_ctx* ctx, const void* x, const void* y, size_t nreal, int prec, double* d_out)
+{
+    if (prec == 4) {
+        const size_t nv = nreal / 4;
+        dot_kernel<float, 1><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const float*)x, (const float*)y, nv, ctx->d_partial, ctx->d_ticket, d_out);
+    } else {
+        const size_t nv = nreal / 2;
+        dot_kernel<double, 1><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const double*)x, (const double*)y, nv, ctx->d_partial, ctx->d_ticket, d_out);
+    }
+    return check_launch(ctx, "redot");
+}
+
+int blas_cg_update(qcd_ctx* ctx, DevScalar a, const void* p, const void* q, void* x, void* r, size_t nreal, int prec,
+                   double* d_out, double* d_beta, const double* d_rho_old)
+{
+    if (prec == 4) {
+        const size_t nv = nreal / 4;
+        cg_update_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const float*)p, (const float*)q, (float*)x, (float*)r, nv,
+                                                                                   ctx->d_partial, ctx->d_ticket, d_out, d_beta, d_rho_old);
+    } else {
+        const size_t nv = nreal / 2;
+        cg_update_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const double*)p, (const double*)q, (double*)x, (double*)r, nv,
+                                                                                    ctx->d_partial, ctx->d_ticket, d_out, d_beta, d_rho_old);
+    }
+    return check_launch(ctx, "cg_update");
+}
+
+int blas_accumulate_hi(qcd_ctx* ctx, void* y_hi, void* x_lo, size_t nreal)
+{
+    const size_t n4 = nreal / 4;
+    accumulate_hi_kernel<<<grid_for(ctx, n4), BLAS_THREADS, 0, ctx->stream>>>((double*)y_hi, (float*)x_lo, n4);
+    return check_launch(ctx, "accumulate_hi");
+}
+
+int blas_residual_hi(qcd_ctx* ctx, void* r_hi, void* r_lo, const void* b, const void* t, size_t nreal, double* d_out)
+{
+    const size_t n4 = nreal / 4;
+    residual_hi_kernel<<<grid_for(ctx, n4), BLAS_THREADS, 0, ctx->stream>>>((double*)r_hi, (float*)r_lo, (const double*)b, (const double*)t, n4,
+                                                                          ctx->d_partial, ctx->d_ticket, d_out);
+    return check_launch(ctx, "residual_hi");
+}
+
+int blas_convert(qcd_ctx* ctx, void* dst, int pdst, const void* src, int psrc, size_t nreal)
+{
+    const int g = grid_for(ctx, nreal);
+    if (pdst == 4 && psrc == 8)
+        convert_kernel<float, double><<<g, BLAS_THREADS, 0, ctx->stream>>>((float*)dst, (const double*)src, nreal);
+    else if (pdst == 8 && psrc == 4)
+        convert_kernel<double, float><<<g, BLAS_THREADS, 0, ctx->stream>>>((double*)dst, (const float*)src, nreal);
+    else if (pdst == 4 && psrc == 4)
+        convert_kernel<float, float><<<g, BLAS_THREADS, 0, ctx->stream>>>((float*)dst, (const float*)src, nreal);
+    else
+        convert_kernel<double, double><<<g, BLAS_THREADS, 0, ctx->stream>>>((double*)dst, (const double*)src, nreal);
+    return check_launch(ctx, "convert");
+}
+
+int blas_zero(qcd_ctx* ctx, void* x, size_t bytes)
+{
+    cudaError_t e = cudaMemsetAsync(x, 0, bytes, ctx->stream);
+    if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "memset: %s", cudaGetErrorString(e));
+    return QCD_OK;
+}
+
+int blas_copy(qcd_ctx* ctx, void* dst, const void* src, size_t bytes)
+{
+    cudaError_t e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, ctx->stream);
+    if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "memcpy: %s", cudaGetErrorString(e));
+    return QCD_OK;
+}

@@ -1,0 +1,314 @@
+/*
+ * clover.cu -- clover term construction (BASELINE.json configs[2]:
+ * "clover field built from the plaquette field-strength F_munu with csw=1.0"; readings
+ * O3/S9 in DESIGN.md).  Setup path: untimed, parity-checked.
+ *
+ *   Q_mn(x)  = sum of the four plaquette leaves in the (m,n) plane around x
+ *   Fhat_mn  = (Q_mn - Q_mn^dag)/8
+ *   A(x)     = 1 + kappa*csw * sum_{m<n} i sigma_mn (x) Fhat_mn(x),  sigma_mn = (i/2)[g_m, g_n]
+ *
+ * sigma_mn is block diagonal in chirality (gamma5 = diag(1,1,-1,-1)), so A is two
+ * Hermitian 6x6 blocks, stored as 6 real diagonal + 15 complex lower entries each.
+ * All arithmetic here is fp64 whatever the storage precision.
+ */
+#include <math.h>
+
+#include "qcd_device.cuh"
+
+namespace {
+
+struct cplx {
+    double re, im;
+};
+__host__ __device__ inline cplx cmul(cplx a, cplx b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+__host__ __device__ inline cplx cadd(cplx a, cplx b) { return {a.re + b.re, a.im + b.im}; }
+__host__ __device__ inline cplx csub(cplx a, cplx b) { return {a.re - b.re, a.im - b.im}; }
+__host__ __device__ inline cplx cconj(cplx a) { return {a.re, -a.im}; }
+
+/* i * sigma_mn, planes (01,02,03,12,13,23), 4x4 each; filled by the host at first use */
+__constant__ cplx c_isigma[6][4][4];
+
+/* DeGrand-Rossi gamma matrices (BASELINE.json configs[0]); entries are 0, +-1, +-i:
+ * code 0 = 0, 1 = +1, 2 = -1, 3 = +i, 4 = -i. */
+const int h_gamma_code[4][4][4] = {
+    /* gamma_x */ {{0, 0, 0, 3}, {0, 0, 3, 0}, {0, 4, 0, 0}, {4, 0, 0, 0}},
+    /* gamma_y */ {{0, 0, 0, 2}, {0, 0, 1, 0}, {0, 1, 0, 0}, {2, 0, 0, 0}},
+    /* gamma_z */ {{0, 0, 3, 0}, {0, 0, 0, 4}, {4, 0, 0, 0}, {0, 3, 0, 0}},
+    /* gamma_t */ {{0, 0, 1, 0}, {0, 0, 0, 1}, {1, 0, 0, 0}, {0, 1, 0, 0}}};
+
+int upload_sigma()
+{
+    static bool done = false;
+    cplx g[4][4][4];
+    const cplx code[5] = {{0, 0}, {1, 0}, {-1, 0}, {0, 1}, {0, -1}};
+    for (int m = 0; m < 4; m++)
+        for (int i = 0; i < 4; i++)
+            for (int j = 0; j < 4; j++) g[m][i][j] = code[h_gamma_code[m][i][j]];
+    cplx is[6][4][4];
+    int pl = 0;
+    for (int m = 0; m < 4; m++)
+        for (int n = m + 1; n < 4; n++, pl++)
+            for (int i = 0; i < 4; i++)
+                for (int j = 0; j < 4; j++) {
+                    cplx c = {0, 0};
+                    for (int k = 0; k < 4; k++) c = cadd(c, csub(cmul(g[m][i][k], g[n][k][j]), cmul(g[n][i][k], g[m][k][j])));
+                    /* sigma = (i/2) [g_m, g_n];  i*sigma = -(1/2)[g_m, g_n] */
+                    is[pl][i][j] = {-0.5 * c.re, -0.5 * c.im};
+                }
+    (void)done;
+    cudaError_t e = cudaMemcpyToSymbol(c_isigma, is, sizeof(is));
+    return e == cudaSuccess ? 0 : -1;
+}
+
+struct M3 {
+    cplx m[9];
+};
+__device__ inline M3 mul(const M3& a, const M3& b)
+{
+    M3 c;
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            cplx s = {0, 0};
+#pragma unroll
+            for (int k = 0; k < 3; k++) s = cadd(s, cmul(a.m[3 * i + k], b.m[3 * k + j]));
+            c.m[3 * i + j] = s;
+        }
+    return c;
+}
+__device__ inline M3 dag(const M3& a)
+{
+    M3 c;
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) c.m[3 * i + j] = cconj(a.m[3 * j + i]);
+    return c;
+}
+
+template <typename T, int RECON> struct LinkReader {
+    const T* data;
+    size_t gblock;
+    DevGeom g;
+    /* U_mu at site c shifted by dm in direction m and dn in direction n (periodic) */
+    __device__ M3 get(int mu, const Coord& c, int m, int dm, int n, int dn) const
+    {
+        int x[4] = {c.x, c.y, c.z, c.t};
+        const int L[4] = {g.X, g.Y, g.Z, g.T};
+        x[m] = (x[m] + dm + L[m]) % L[m];
+        x[n] = (x[n] + dn + L[n]) % L[n];
+        const int parity = (x[0] + x[1] + x[2] + x[3]) & 1;
+        const int cb = coord_to_cb(g, x[0], x[1], x[2], x[3]);
+        T u[18];
+        load_link<T, RECON>(u, data + (size_t)(2 * mu + parity) * gblock, (size_t)g.Vh, (size_t)cb);
+        M3 r;
+#pragma unroll
+        for (int k = 0; k < 9; k++) r.m[k] = {(double)u[2 * k], (double)u[2 * k + 1]};
+        return r;
+    }
+};
+
+__device__ inline int tri_index(int hi, int lo) { return 5 * lo - (lo * (lo - 1)) / 2 + (hi - lo - 1); }
+
+/* in-place inverse of a 6x6 complex matrix, Gauss-Jordan with partial pivoting */
+__device__ bool invert6(cplx (*a)[6])
+{
+    cplx inv[6][6];
+    for (int i = 0; i < 6; i++)
+        for (int j = 0; j < 6; j++) inv[i][j] = {i == j ? 1.0 : 0.0, 0.0};
+    for (int col = 0; col < 6; col++) {
+        int piv = col;
+        double best = a[col][col].re * a[col][col].re + a[col][col].im * a[col][col].im;
+        for (int r = col + 1; r < 6; r++) {
+            const double v = a[r][col].re * a[r][col].re + a[r][col].im * a[r][col].im;
+            if (v > best) { best = v; piv = r; }
+        }
+        if (!(best > 0.0)) return false;
+        if (piv != col)
+            for (int j = 0; j < 6; j++) {
+                cplx t = a[col][j]; a[col][j] = a[piv][j]; a[piv][j] = t;
+                t = inv[col][j]; inv[col][j] = inv[piv][j]; inv[piv][j] = t;
+            }
+        const cplx p = a[col][col];
+        const double d = p.re * p.re + p.im * p.im;
+        const cplx pinv = {p.re / d, -p.im / d};
+        for (int j = 0; j < 6; j++) {
+            a[col][j] = cmul(a[col][j], pinv);
+            inv[col][j] = cmul(inv[col][j], pinv);
+        }
+        for (int r = 0; r < 6; r++) {
+            if (r == col) continue;
+            const cplx f = a[r][col];
+            for (int j = 0; j < 6; j++) {
+                a[r][j] = csub(a[r][j], cmul(f, a[col][j]));
+                inv[r][j] = csub(inv[r][j], cmul(f, inv[col][j]));
+            }
+        }
+    }
+    for (int i = 0; i < 6; i++)
+        for (int j = 0; j < 6; j++) a[i][j] = inv[i][j];
+    return true;
+}
+
+template <typename TS> __device__ void store_block(TS* blk, size_t Vh, size_t cb, int b, cplx (*a)[6])
+{
+    TS r[36];
+    for (int i = 0; i < 6; i++) r[i] = (TS)a[i][i].re;
+    for (int lo = 0; lo < 6; lo++)
+        for (int hi = lo + 1; hi < 6; hi++) {
+            const int k = 6 + 2 * tri_index(hi, lo);
+            /* Hermitian by construction; store the Hermitian part of the pair */
+            r[k] = (TS)(0.5 * (a[hi][lo].re + a[lo][hi].re));
+            r[k + 1] = (TS)(0.5 * (a[hi][lo].im - a[lo][hi].im));
+        }
+    store_planes<TS, 36>(blk + (size_t)36 * b * Vh, Vh, cb, r);
+}
+
+template <typename T, int RECON, typename TS>
+__global__ void __launch_bounds__(64) clover_build_kernel(LinkReader<T, RECON> R, TS* A, TS* Ainv, size_t cblock, double coeff, int* bad)
+{
+    const DevGeom& g = R.g;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * g.Vh) return;
+    const int parity = i / g.Vh, cb = i - parity * g.Vh;
+    const Coord c = cb_to_coord(g, cb, parity);
+
+    cplx blk[2][6][6];
+    for (int b = 0; b < 2; b++)
+        for (int r = 0; r < 6; r++)
+            for (int s = 0; s < 6; s++) blk[b][r][s] = {0.0, 0.0};
+
+    int pl = 0;
+    for (int m = 0; m < 4; m++)
+        for (int n = m + 1; n < 4; n++, pl++) {
+            /* the four leaves, each a closed loop x -> ... -> x, counter-clockwise in (m,n) */
+            M3 q = mul(mul(R.get(m, c, m, 0, n, 0), R.get(n, c, m, 1, n, 0)),
+                       mul(dag(R.get(m, c, m, 0, n, 1)), dag(R.get(n, c, m, 0, n, 0))));
+            M3 l = mul(mul(R.get(n, c, m, 0, n, 0), dag(R.get(m, c, m, -1, n, 1))),
+                       mul(dag(R.get(n, c, m, -1, n, 0)), R.get(m, c, m, -1, n, 0)));
+            for (int k = 0; k < 9; k++) q.m[k] = cadd(q.m[k], l.m[k]);
+            l = mul(mul(dag(R.get(m, c, m, -1, n, 0)), dag(R.get(n, c, m, -1, n, -1))),
+                    mul(R.get(m, c, m, -1, n, -1), R.get(n, c, m, 0, n, -1)));
+            for (int k = 0; k < 9; k++) q.m[k] = cadd(q.m[k], l.m[k]);
+            l = mul(mul(dag(R.get(n, c, m, 0, n, -1)), R.get(m, c, m, 0, n, -1)),
+                    mul(R.get(n, c, m, 1, n, -1), dag(R.get(m, c, m, 0, n, 0))));
+            for (int k = 0; k < 9; k++) q.m[k] = cadd(q.m[k], l.m[k]);
+            /* Fhat = (Q - Q^dag)/8 */
+            M3 f;
+            for (int a = 0; a < 3; a++)
+                for (int bb = 0; bb < 3; bb++) {
+                    const cplx d = csub(q.m[3 * a + bb], cconj(q.m[3 * bb + a]));
+                    f.m[3 * a + bb] = {0.125 * d.re, 0.125 * d.im};
+                }
+            /* C += (i sigma_mn) (x) Fhat, chirality block by block */
+            for (int b = 0; b < 2; b++)
+                for (int s = 0; s < 2; s++)
+                    for (int sp = 0; sp < 2; sp++) {
+                        const cplx sg = c_isigma[pl][2 * b + s][2 * b + sp];
+                        if (sg.re == 0.0 && sg.im == 0.0) continue;
+                        for (int a = 0; a < 3; a++)
+                            for (int bb = 0; bb < 3; bb++)
+                                blk[b][3 * s + a][3 * sp + bb] = cadd(blk[b][3 * s + a][3 * sp + bb], cmul(sg, f.m[3 * a + bb]));
+                    }
+        }
+
+    for (int b = 0; b < 2; b++) {
+        for (int r = 0; r < 6; r++)
+            for (int s = 0; s < 6; s++) {
+                blk[b][r][s].re *= coeff;
+                blk[b][r][s].im *= coeff;
+                if (r == s) blk[b][r][s].re += 1.0;
+            }
+        store_block<TS>(A + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, b, blk[b]);
+        if (!invert6(blk[b])) atomicAdd(bad, 1);
+        store_block<TS>(Ainv + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, b, blk[b]);
+    }
+}
+
+/* expand packed blocks to dense 12x12 complex per site, boundary site order, fp64 */
+template <typename TS> __global__ void clover_unpack_kernel(double* dense, const TS* C, size_t cblock, DevGeom g)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * g.Vh) return;
+    const int parity = i / g.Vh, cb = i - parity * g.Vh;
+    const Coord c = cb_to_coord(g, cb, parity);
+    const size_t s = (size_t)c.x + (size_t)g.X * (c.y + (size_t)g.Y * (c.z + (size_t)g.Z * c.t));
+    double* d = dense + s * 288;
+    for (int k = 0; k < 288; k++) d[k] = 0.0;
+    for (int b = 0; b < 2; b++) {
+        TS r[36];
+        load_planes_rw<TS, 36>(r, C + (size_t)parity * cblock + (size_t)36 * b * g.Vh, (size_t)g.Vh, (size_t)cb);
+        for (int ii = 0; ii < 6; ii++) {
+            const int row = 6 * b + ii;
+            d[(row * 12 + row) * 2] = (double)r[ii];
+            for (int jj = 0; jj < ii; jj++) {
+                const int col = 6 * b + jj;
+                const int k = 6 + 2 * tri_index(ii, jj);
+                d[(row * 12 + col) * 2] = (double)r[k];
+                d[(row * 12 + col) * 2 + 1] = (double)r[k + 1];
+                d[(col * 12 + row) * 2] = (double)r[k];
+                d[(col * 12 + row) * 2 + 1] = -(double)r[k + 1];
+            }
+        }
+    }
+}
+
+template <typename T, int RECON>
+cudaError_t build_launch(qcd_ctx* ctx, const qcd_gauge* gh, const qcd_clover* c, int* d_bad)
+{
+    LinkReader<T, RECON> R;
+    R.data = (const T*)gh->data;
+    R.gblock = gh->block_bytes / sizeof(T);
+    R.g = dev_geom(gh->geo);
+    const int threads = 64, blocks = (2 * R.g.Vh + threads - 1) / threads;
+    const double coeff = c->kappa * c->csw;
+    if (c->precision == 4) {
+        const size_t cblock = c->block_bytes / 4;
+        float* A = (float*)c->data;
+        clover_build_kernel<T, RECON, float><<<blocks, threads, 0, ctx->stream>>>(R, A, A + 2 * cblock, cblock, coeff, d_bad);
+    } else {
+        const size_t cblock = c->block_bytes / 8;
+        double* A = (double*)c->data;
+        clover_build_kernel<T, RECON, double><<<blocks, threads, 0, ctx->stream>>>(R, A, A + 2 * cblock, cblock, coeff, d_bad);
+    }
+    return cudaGetLastError();
+}
+
+} // namespace
+
+int clover_build(qcd_ctx* ctx, const qcd_gauge* g, const qcd_clover* c)
+{
+    if (upload_sigma() != 0) return qcd_set_error(QCD_ECUDA, "clover: constant upload failed");
+    int* d_bad = reinterpret_cast<int*>(ctx->d_ticket + 8);
+    QCD_CHECK_CUDA(cudaMemsetAsync(d_bad, 0, sizeof(int), ctx->stream));
+    cudaError_t e;
+    if (g->precision == 4)
+        e = (g->reconstruct == 12) ? build_launch<float, 12>(ctx, g, c, d_bad) : build_launch<float, 18>(ctx, g, c, d_bad);
+    else
+        e = (g->reconstruct == 12) ? build_launch<double, 12>(ctx, g, c, d_bad) : build_launch<double, 18>(ctx, g, c, d_bad);
+    if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "clover build: %s", cudaGetErrorString(e));
+    ctx->launches++;
+    int bad = 0;
+    QCD_CHECK_CUDA(cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    QCD_CHECK_CUDA(cudaStreamSynchronize(ctx->stream));
+    if (bad) return qcd_set_error(QCD_EBREAKDOWN, "clover: %d singular 6x6 blocks", bad);
+    return QCD_OK;
+}
+
+int clover_unpack(qcd_ctx* ctx, void* dense, const qcd_clover* c, int which)
+{
+    const DevGeom g = dev_geom(c->geo);
+    const int threads = 64, blocks = (2 * g.Vh + threads - 1) / threads;
+    if (c->precision == 4) {
+        const size_t cblock = c->block_bytes / 4;
+        clover_unpack_kernel<float><<<blocks, threads, 0, ctx->stream>>>((double*)dense, (const float*)c->data + (which ? 2 * cblock : 0), cblock, g);
+    } else {
+        const size_t cblock = c->block_bytes / 8;
+        clover_unpack_kernel<double><<<blocks, threads, 0, ctx->stream>>>((double*)dense, (const double*)c->data + (which ? 2 * cblock : 0), cblock, g);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "clover unpack: %s", cudaGetErrorString(e));
+    ctx->launches++;
+    return QCD_OK;
+}

@@ -1,0 +1,8 @@
+/* fp32 instantiations of the hopping-term kernel (single precision). */
+#include "hop_kernel.cuh"
+
+cudaError_t hop_launch_f32(const qcd_gauge* g, const HopLaunch& L, cudaStream_t st)
+{
+    HopArgs<float> A = make_hop_args<float>(g, L);
+    return hop_dispatch<float>(A, g->reconstruct, L.dagger, L.mode, st);
+}

@@ -1,0 +1,166 @@
+/*
+ * qcd_device.cuh -- device helpers: 128-bit field access, checkerboard indexing,
+ * SU(3) link loading with 12-real reconstruction (links "suppressed to
+ * 12 real numbers to save the memory bandwidth").
+ */
+#ifndef QCD_DEVICE_CUH
+#define QCD_DEVICE_CUH
+
+#include "qcd_internal.h"
+
+template <typename T> struct Vec;
+template <> struct Vec<float> {
+    typedef float4 type;
+    static constexpr int reals = 4;
+};
+template <> struct Vec<double> {
+    typedef double2 type;
+    static constexpr int reals = 2;
+};
+
+/* number of 128-bit chunks holding n reals */
+template <typename T> __host__ __device__ constexpr int chunks_of(int nreal)
+{
+    return nreal / Vec<T>::reals;
+}
+
+__device__ __forceinline__ void vec_get(const float4& v, float* d)
+{
+    d[0] = v.x; d[1] = v.y; d[2] = v.z; d[3] = v.w;
+}
+__device__ __forceinline__ void vec_get(const double2& v, double* d)
+{
+    d[0] = v.x; d[1] = v.y;
+}
+__device__ __forceinline__ float4 vec_make(const float* d) { return make_float4(d[0], d[1], d[2], d[3]); }
+__device__ __forceinline__ double2 vec_make(const double* d) { return make_double2(d[0], d[1]); }
+
+/* load / store NREAL reals of site idx from a [chunk][stride] plane array */
+template <typename T, int NREAL>
+__device__ __forceinline__ void load_planes(T (&d)[NREAL], const T* __restrict__ base, size_t stride,
+                                            size_t idx)
+{
+    typedef typename Vec<T>::type V;
+    const V* p = reinterpret_cast<const V*>(base) + idx;
+#pragma unroll
+    for (int c = 0; c < NREAL / Vec<T>::reals; c++) {
+        V v = __ldg(p + (size_t)c * stride);
+        vec_get(v, &d[c * Vec<T>::reals]);
+    }
+}
+/* plain (coherent) load: for buffers that the same kernel also writes elsewhere */
+template <typename T, int NREAL>
+__device__ __forceinline__ void load_planes_rw(T (&d)[NREAL], const T* base, size_t stride, size_t idx)
+{
+    typedef typename Vec<T>::type V;
+    const V* p = reinterpret_cast<const V*>(base) + idx;
+#pragma unroll
+    for (int c = 0; c < NREAL / Vec<T>::reals; c++) {
+        V v = p[(size_t)c * stride];
+        vec_get(v, &d[c * Vec<T>::reals]);
+    }
+}
+template <typename T, int NREAL>
+__device__ __forceinline__ void store_planes(T* base, size_t stride, size_t idx, const T (&d)[NREAL])
+{
+    typedef typename Vec<T>::type V;
+    V* p = reinterpret_cast<V*>(base) + idx;
+#pragma unroll
+    for (int c = 0; c < NREAL / Vec<T>::reals; c++) p[(size_t)c * stride] = vec_make(&d[c * Vec<T>::reals]);
+}
+
+/* ---- SU(3) link: u[2*(3*row+col)+reim] ------------------------------------------ */
+/* row2 = conj(row0 x row1)  (reading S7) */
+template <typename T> __device__ __forceinline__ void reconstruct_row2(T (&u)[18])
+{
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+        /* (r0 x r1)_c = r0[c1] r1[c2] - r0[c2] r1[c1] */
+        const T ar = u[2 * c1], ai = u[2 * c1 + 1], br = u[6 + 2 * c2], bi = u[6 + 2 * c2 + 1];
+        const T cr = u[2 * c2], ci = u[2 * c2 + 1], dr = u[6 + 2 * c1], di = u[6 + 2 * c1 + 1];
+        const T re = ar * br - ai * bi - (cr * dr - ci * di);
+        const T im = ar * bi + ai * br - (cr * di + ci * dr);
+        u[12 + 2 * c] = re;
+        u[12 + 2 * c + 1] = -im;
+    }
+}
+
+/* block = base of one (mu, parity) gauge block; Vh sites */
+template <typename T, int RECON>
+__device__ __forceinline__ void load_link(T (&u)[18], const T* __restrict__ block, size_t Vh, size_t cb)
+{
+    if (RECON == 12) {
+        T r[12];
+        load_planes<T, 12>(r, block, Vh, cb);
+#pragma unroll
+        for (int i = 0; i < 12; i++) u[i] = r[i];
+        reconstruct_row2<T>(u);
+    } else if (sizeof(T) == 8) {
+        load_planes<T, 18>(u, block, Vh, cb);
+    } else {
+        /* fp32 18-real: 4 float4 planes then one float2 plane */
+        T r[16];
+        load_planes<T, 16>(r, block, Vh, cb);
+#pragma unroll
+        for (int i = 0; i < 16; i++) u[i] = r[i];
+        const float2* tail = reinterpret_cast<const float2*>(block + 16 * Vh) + cb;
+        const float2 v = __ldg(tail);
+        u[16] = (T)v.x;
+        u[17] = (T)v.y;
+    }
+}
+
+template <typename T, int RECON>
+__device__ __forceinline__ void store_link(T* block, size_t Vh, size_t cb, const T (&u)[18])
+{
+    if (RECON == 12) {
+        T r[12];
+#pragma unroll
+        for (int i = 0; i < 12; i++) r[i] = u[i];
+        store_planes<T, 12>(block, Vh, cb, r);
+    } else if (sizeof(T) == 8) {
+        store_planes<T, 18>(block, Vh, cb, u);
+    } else {
+        T r[16];
+#pragma unroll
+        for (int i = 0; i < 16; i++) r[i] = u[i];
+        store_planes<T, 16>(block, Vh, cb, r);
+        float2* tail = reinterpret_cast<float2*>(block + 16 * Vh) + cb;
+        *tail = make_float2((float)u[16], (float)u[17]);
+    }
+}
+
+/* ---- checkerboard indexing (reading S3) -------------------------------------------
+ * lexicographic s = x + X (y + Y (z + Z t)); parity = (x+y+z+t)&1; cb = s >> 1. */
+struct DevGeom {
+    int X, Y, Z, T, X2, Vh;
+};
+static inline DevGeom dev_geom(const Geom& g)
+{
+    DevGeom d = {g.X, g.Y, g.Z, g.T, g.X2, g.Vh};
+    return d;
+}
+
+struct Coord {
+    int x, y, z, t;
+};
+__device__ __forceinline__ Coord cb_to_coord(const DevGeom& g, int cb, int parity)
+{
+    Coord c;
+    unsigned r = (unsigned)cb;
+    const unsigned xh = r % (unsigned)g.X2;
+    r /= (unsigned)g.X2;
+    c.y = (int)(r % (unsigned)g.Y);
+    r /= (unsigned)g.Y;
+    c.z = (int)(r % (unsigned)g.Z);
+    c.t = (int)(r / (unsigned)g.Z);
+    c.x = 2 * (int)xh + ((c.y + c.z + c.t + parity) & 1);
+    return c;
+}
+__device__ __forceinline__ int coord_to_cb(const DevGeom& g, int x, int y, int z, int t)
+{
+    return (x + g.X * (y + g.Y * (z + g.Z * t))) >> 1;
+}
+
+#endif

@@ -1,0 +1,157 @@
+/*
+ * qcd_internal.h -- host-side structures shared by the translation units of
+ * libqcd_b200.so (CUDA path only; nothing here is used by oracle/).
+ *
+ * Field layouts in HBM (include/qcd.h "Conventions"):
+ *   spinor, one parity : [chunk][cb]            chunk = one 128-bit word
+ *                        fp32: 6 x float4 (2 complex each), fp64: 12 x double2
+ *   gauge              : [mu][parity][chunk][cb]
+ *                        12-real: 3 float4 / 6 double2 (rows 0,1)
+ *                        18-real: fp32 4 float4 + 1 float2 plane, fp64 9 double2
+ *   clover (A, A^-1)   : [which][parity][chunk][cb], 72 reals = 18 float4 / 36 double2
+ *                        per site: chirality block b=0,1 -> 6 real diagonal then the
+ *                        15 complex strictly-lower entries, column by column.
+ */
+#ifndef QCD_INTERNAL_H
+#define QCD_INTERNAL_H
+
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/qcd.h"
+
+struct Geom {
+    int X, Y, Z, T;   /* full dims                       */
+    int X2;           /* X/2                             */
+    int Vh;           /* sites per parity                */
+    long long V;
+};
+
+struct qcd_ctx {
+    int device;
+    cudaStream_t stream;
+    void* ws;
+    size_t ws_bytes;
+    double* d_partial;      /* block partial sums (device)                 */
+    unsigned int* d_ticket; /* last-block tickets, one per reduction slot  */
+    double* d_scalar;       /* device-resident CG scalars                  */
+    double* h_scalar;       /* pinned host mirror                          */
+    int max_blocks;
+    int num_sms;
+    long long launches;
+    /* operator selected by qcd_set_operator */
+    const qcd_gauge *g_hi, *g_lo;
+    const qcd_clover *c_hi, *c_lo;
+    double kappa, csw, delta;
+    int op_parity;
+    int op_set;
+};
+
+struct qcd_gauge {
+    qcd_ctx* ctx;
+    Geom geo;
+    int precision;    /* 4 | 8   */
+    int reconstruct;  /* 12 | 18 */
+    int tb;           /* +1 | -1 */
+    void* data;
+    size_t block_bytes; /* bytes of one (mu, parity) block */
+};
+
+struct qcd_clover {
+    qcd_ctx* ctx;
+    Geom geo;
+    int precision;
+    double kappa, csw;
+    void* data;          /* A[parity 0], A[parity 1], Ainv[parity 0], Ainv[parity 1] */
+    size_t block_bytes;  /* bytes of one parity block = Vh * 72 * precision          */
+};
+
+/* device scalar slots (doubles) used by the solvers */
+enum { SC_RHO = 0, SC_PQ = 1, SC_RHO_NEW = 2, SC_BETA = 3, SC_TMP = 4, SC_COUNT = 16 };
+
+int qcd_set_error(int code, const char* fmt, ...);
+#define QCD_CHECK_CUDA(expr)                                                          \
+    do {                                                                              \
+        cudaError_t e__ = (expr);                                                     \
+        if (e__ != cudaSuccess)                                                       \
+            return qcd_set_error(QCD_ECUDA, "%s: %s (%s:%d)", #expr,                  \
+                                 cudaGetErrorString(e__), __FILE__, __LINE__);        \
+    } while (0)
+#define QCD_REQUIRE(cond, ...)                                                        \
+    do {                                                                              \
+        if (!(cond)) return qcd_set_error(QCD_EINVAL, __VA_ARGS__);                   \
+    } while (0)
+
+/* ---- hop launch description (hop.cu) ------------------------------------------- */
+enum HopMode {
+    HOP_PLAIN = 0,       /* out = H in                                            */
+    HOP_XPAY = 1,        /* out = a z + b H in                                    */
+    HOP_CLOVER_Z = 2,    /* out = a (A z) + b H in                                */
+    HOP_CLOVER_OUT = 3,  /* out = Ainv (H in)                                     */
+    HOP_CHEB = 4         /* tn = c1 g5 (z + b H in) + c2 tm; y (+)= ck tn; tm = tn */
+};
+
+struct HopLaunch {
+    void* out;            /* one-parity block (cheb: unused)                      */
+    const void* in;       /* other-parity block                                   */
+    const void* z;        /* own-parity block (modes 1,2,4)                       */
+    void* y;              /* cheb accumulator, own parity                         */
+    void* tm;             /* cheb T_{k-1} in / T_{k+1} out, own parity            */
+    const void* clover;   /* A or A^-1 block of the output parity (modes 2,3)     */
+    double a, b, c1, c2, ck;
+    int y_init;           /* cheb: y = c0 z + ck tn instead of y += ck tn         */
+    double c0;
+    int out_parity, dagger, mode;
+};
+
+int hop_launch(qcd_ctx* ctx, const qcd_gauge* g, const HopLaunch& L);
+
+/* out = M in (or M^dag in): parity 2 = (A - kappa H) on the full lattice (two launches);
+ * parity 0|1 = even-odd Schur operator on that parity (two launches, tmp = one parity block). */
+int op_apply_M(qcd_ctx* ctx, void* out, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c,
+               double kappa, int parity, int dagger);
+
+/* ---- blas.cu --------------------------------------------------------------------- */
+/* A scalar that is either a host value or the quotient of two device doubles. */
+struct DevScalar {
+    double val;
+    const double* num;
+    const double* den;
+    double sign;
+};
+static inline DevScalar host_scalar(double v) { DevScalar s = {v, nullptr, nullptr, 1.0}; return s; }
+static inline DevScalar dev_ratio(const double* n, const double* d, double sign = 1.0)
+{
+    DevScalar s = {0.0, n, d, sign};
+    return s;
+}
+
+int blas_axpby(qcd_ctx*, DevScalar a, const void* x, DevScalar b, void* y, size_t nreal, int prec);
+int blas_norm2(qcd_ctx*, const void* x, size_t nreal, int prec, double* d_out);
+int blas_redot(qcd_ctx*, const void* x, const void* y, size_t nreal, int prec, double* d_out);
+/* x += a p; r -= a q; *d_out = |r|^2; if d_beta: *d_beta = |r|^2 / *d_rho_old */
+int blas_cg_update(qcd_ctx*, DevScalar a, const void* p, const void* q, void* x, void* r,
+                   size_t nreal, int prec, double* d_out, double* d_beta, const double* d_rho_old);
+/* y(hi) += x(lo); x = 0 */
+int blas_accumulate_hi(qcd_ctx*, void* y_hi, void* x_lo, size_t nreal);
+/* r_hi = b - t (fp64); r_lo = (float) r_hi; *d_out = |r_hi|^2 */
+int blas_residual_hi(qcd_ctx*, void* r_hi, void* r_lo, const void* b, const void* t, size_t nreal,
+                     double* d_out);
+int blas_convert(qcd_ctx*, void* dst, int pdst, const void* src, int psrc, size_t nreal);
+int blas_zero(qcd_ctx*, void* x, size_t bytes);
+int blas_copy(qcd_ctx*, void* dst, const void* src, size_t bytes);
+
+int layout_spinor_pack(qcd_ctx*, void* internal, const void* boundary, const Geom&, int prec, int unpack);
+int layout_gauge_load(qcd_ctx*, const qcd_gauge* g, const void* links, int prec_in);
+
+/* ---- clover.cu -------------------------------------------------------------------- */
+int clover_build(qcd_ctx*, const qcd_gauge* g, const qcd_clover* c);
+int clover_unpack(qcd_ctx*, void* dense, const qcd_clover* c, int which);
+
+static inline size_t gauge_block_bytes(const Geom& g, int precision, int reconstruct)
+{
+    return (size_t)g.Vh * (size_t)reconstruct * (size_t)precision;
+}
+
+#endif

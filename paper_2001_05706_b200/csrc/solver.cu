@@ -1,0 +1,317 @@
+/*
+ * solver.cu -- CG on N = M^dag M (reading O6/S13), the
+ * reliable-update mixed-precision CG (a12, reading O7/S15; PAPER.md:163 ref. [1]) and
+ * the Chebyshev polynomial driver (a14, reading O8/S16).
+ *
+ * alpha and beta never leave the device: reductions write rho, <p,Np> and beta to
+ * device slots and the update kernels read them there.  The host reads back two
+ * doubles per iteration for the stopping test.
+ */
+#include <math.h>
+#include <string.h>
+
+#include "qcd_internal.h"
+
+namespace {
+
+qcd_ctx* g_last_ctx = nullptr;
+
+/* device scalar slots */
+enum { S_RHO_A = 0, S_RHO_B = 1, S_PQ = 2, S_BETA = 3, S_ONE = 5, S_AUX = 6 };
+
+struct Op {
+    qcd_ctx* ctx;
+    const qcd_gauge* g;
+    const qcd_clover* c;
+    double kappa;
+    int parity;
+    size_t nreal;
+    size_t bytes;
+};
+
+Op make_op(qcd_ctx* ctx, const qcd_gauge* g, const qcd_clover* c)
+{
+    Op o;
+    o.ctx = ctx; o.g = g; o.c = c; o.kappa = ctx->kappa; o.parity = ctx->op_parity;
+    o.nreal = (size_t)(ctx->op_parity == 2 ? g->geo.V : g->geo.Vh) * 24;
+    o.bytes = o.nreal * g->precision;
+    return o;
+}
+
+/* q = M^dag M p, t = M p (kept), tmp = hop temporary */
+int apply_N(const Op& o, void* q, const void* p, void* t, void* tmp)
+{
+    int rc = op_apply_M(o.ctx, t, p, tmp, o.g, o.c, o.kappa, o.parity, 0);
+    if (rc) return rc;
+    return op_apply_M(o.ctx, q, t, tmp, o.g, o.c, o.kappa, o.parity, 1);
+}
+
+int fetch(qcd_ctx* ctx, int slot, int n)
+{
+    QCD_CHECK_CUDA(cudaMemcpyAsync(ctx->h_scalar + slot, ctx->d_scalar + slot, sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream));
+    QCD_CHECK_CUDA(cudaStreamSynchronize(ctx->stream));
+    return QCD_OK;
+}
+
+int set_one(qcd_ctx* ctx)
+{
+    ctx->h_scalar[S_ONE] = 1.0;
+    QCD_CHECK_CUDA(cudaMemcpyAsync(ctx->d_scalar + S_ONE, ctx->h_scalar + S_ONE, sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    return QCD_OK;
+}
+
+#define RC(expr)               \
+    do {                       \
+        int rc__ = (expr);     \
+        if (rc__) return rc__; \
+    } while (0)
+
+int true_residual(const Op& o, const void* x, const void* b, void* q, void* t, void* tmp, double bnorm, double* r_true)
+{
+    qcd_ctx* ctx = o.ctx;
+    const int P = o.g->precision;
+    RC(apply_N(o, q, x, t, tmp));
+    RC(blas_axpby(ctx, host_scalar(1.0), b, host_scalar(-1.0), q, o.nreal, P)); /* q = b - q */
+    RC(blas_norm2(ctx, q, o.nreal, P, ctx->d_scalar + S_AUX));
+    RC(fetch(ctx, S_AUX, 1));
+    *r_true = bnorm > 0 ? sqrt(ctx->h_scalar[S_AUX]) / bnorm : 0.0;
+    return QCD_OK;
+}
+
+int cg_pure(qcd_ctx* ctx, void* x, const void* b, double tol, int maxiter, qcd_stats* st)
+{
+    const Op o = make_op(ctx, ctx->g_hi, ctx->c_hi);
+    const int P = o.g->precision;
+    const int nfields = o.parity == 2 ? 4 : 5;
+    QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= nfields * o.bytes, "cg: workspace too small (need %zu bytes)", nfields * o.bytes);
+    char* w = (char*)ctx->ws;
+    void *r = w, *p = w + o.bytes, *q = w + 2 * o.bytes, *t = w + 3 * o.bytes, *tmp = w + 4 * o.bytes;
+    double* d = ctx->d_scalar;
+    double* h = ctx->h_scalar;
+
+    RC(set_one(ctx));
+    RC(blas_zero(ctx, x, o.bytes));
+    RC(blas_copy(ctx, r, b, o.bytes));
+    RC(blas_copy(ctx, p, b, o.bytes));
+    int cur = S_RHO_A, nxt = S_RHO_B;
+    RC(blas_norm2(ctx, b, o.nreal, P, d + cur));
+    RC(fetch(ctx, cur, 1));
+    const double bnorm = sqrt(h[cur]);
+    double rnorm = bnorm;
+    int k = 0, conv = (bnorm == 0.0), brk = 0;
+    while (!conv && k < maxiter) {
+        k++;
+        RC(apply_N(o, q, p, t, tmp));
+        RC(blas_redot(ctx, p, q, o.nreal, P, d + S_PQ));
+        RC(blas_cg_update(ctx, dev_ratio(d + cur, d + S_PQ), p, q, x, r, o.nreal, P, d + nxt, d + S_BETA, d + cur));
+        RC(fetch(ctx, 0, 4));
+        if (!(h[S_PQ] > 0.0)) { brk = 1; break; }
+        rnorm = sqrt(h[nxt]);
+        if (rnorm <= tol * bnorm) { conv = 1; break; }
+        RC(blas_axpby(ctx, host_scalar(1.0), r, dev_ratio(d + S_BETA, d + S_ONE), p, o.nreal, P)); /* p = r + beta p */
+        const int s = cur; cur = nxt; nxt = s;
+    }
+    double r_true = 0.0;
+    RC(true_residual(o, x, b, q, t, tmp, bnorm, &r_true));
+    if (st) {
+        st->iters = k; st->reliable_updates = 0; st->converged = conv; st->breakdown = brk;
+        st->r_iter = bnorm > 0 ? rnorm / bnorm : 0.0;
+        st->r_true = r_true;
+    }
+    if (brk) return qcd_set_error(QCD_EBREAKDOWN, "cg: <p,Np> <= 0 or NaN at iteration %d", k);
+    return conv ? QCD_OK : QCD_NOCONV;
+}
+
+int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_stats* st)
+{
+    const Op oh = make_op(ctx, ctx->g_hi, ctx->c_hi);
+    const Op ol = make_op(ctx, ctx->g_lo, ctx->c_lo);
+    QCD_REQUIRE(oh.g->precision == 8 && ol.g->precision == 4, "mixed cg: needs an fp64 high and an fp32 low operator");
+    const size_t need = 4 * oh.bytes + 6 * ol.bytes;
+    QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= need, "mixed cg: workspace too small (need %zu bytes)", need);
+    char* w = (char*)ctx->ws;
+    void *rh = w, *th = w + oh.bytes, *h1 = w + 2 * oh.bytes, *h2 = w + 3 * oh.bytes;
+    char* wl = w + 4 * oh.bytes;
+    void *x = wl, *r = wl + ol.bytes, *p = wl + 2 * ol.bytes, *q = wl + 3 * ol.bytes, *tl = wl + 4 * ol.bytes, *l2 = wl + 5 * ol.bytes;
+    double* d = ctx->d_scalar;
+    double* h = ctx->h_scalar;
+    const size_t n = oh.nreal;
+
+    RC(set_one(ctx));
+    RC(blas_zero(ctx, y, oh.bytes));
+    RC(blas_zero(ctx, x, ol.bytes));
+    RC(blas_convert(ctx, r, 4, b, 8, n));
+    RC(blas_copy(ctx, p, r, ol.bytes));
+    int cur = S_RHO_A, nxt = S_RHO_B;
+    RC(blas_norm2(ctx, b, n, 8, d + S_AUX));
+    RC(blas_norm2(ctx, r, n, 4, d + cur));
+    RC(fetch(ctx, 0, 8));
+    const double bnorm = sqrt(h[S_AUX]);
+    double rho = h[cur];
+    double rmax = sqrt(rho), rhnorm = bnorm;
+    int k = 0, conv = (bnorm == 0.0), brk = 0, nup = 0;
+    while (!conv && k < maxiter) {
+        k++;
+        RC(apply_N(ol, q, p, tl, l2));
+        RC(blas_redot(ctx, p, q, n, 4, d + S_PQ));
+        RC(blas_cg_update(ctx, dev_ratio(d + cur, d + S_PQ), p, q, x, r, n, 4, d + nxt, nullptr, nullptr));
+        RC(fetch(ctx, 0, 4));
+        if (!(h[S_PQ] > 0.0)) { brk = 1; break; }
+        double rho2 = h[nxt];
+        const double rnorm = sqrt(rho2);
+        if (rnorm > rmax) rmax = rnorm;
+        if (rnorm < ctx->delta * rmax || rnorm <= tol * bnorm) {
+            RC(blas_accumulate_hi(ctx, y, x, n));                 /* y += x ; x = 0          */
+            RC(apply_N(oh, th, y, h1, h2));                       /* th = N_hi y             */
+            RC(blas_residual_hi(ctx, rh, r, b, th, n, d + nxt));  /* rh = b - th ; r = (f)rh */
+            RC(fetch(ctx, nxt, 1));
+            rho2 = h[nxt];
+            rhnorm = sqrt(rho2);
+            rmax = rhnorm;
+            nup++;
+            if (rhnorm <= tol * bnorm) { conv = 1; break; }
+        }
+        const float beta = (float)(rho2 / rho);
+        RC(blas_axpby(ctx, host_scalar(1.0), r, host_scalar((double)beta), p, n, 4));
+        rho = rho2;
+        const int s = cur; cur = nxt; nxt = s;
+    }
+    if (!conv) RC(blas_accumulate_hi(ctx, y, x, n));
+    double r_true = 0.0;
+    RC(true_residual(oh, y, b, th, h1, h2, bnorm, &r_true));
+    if (st) {
+        st->iters = k; st->reliable_updates = nup; st->converged = conv; st->breakdown = brk;
+        st->r_iter = bnorm > 0 ? rhnorm / bnorm : 0.0;
+        st->r_true = r_true;
+    }
+    if (brk) return qcd_set_error(QCD_EBREAKDOWN, "mixed cg: <p,Np> <= 0 or NaN at iteration %d", k);
+    return conv ? QCD_OK : QCD_NOCONV;
+}
+
+double hop_flops_per_apply_M(const Op& o)
+{
+    /* nominal (reading S18): 1320 per output site per hop, +504 per clover / clover-inverse apply */
+    const double Vh = (double)o.g->geo.Vh;
+    const double hops = 2.0; /* both forms launch two single-parity hops per M */
+    double f = hops * 1320.0 * Vh;
+    if (o.c) f += 2.0 * 504.0 * Vh;
+    return f;
+}
+
+} // namespace
+
+extern "C" {
+
+int qcd_set_operator(qcd_ctx* ctx, const qcd_gauge* g_hi, const qcd_gauge* g_lo, const qcd_clover* c_hi, const qcd_clover* c_lo,
+                     double kappa, double csw, int parity, double delta)
+{
+    QCD_REQUIRE(ctx && g_hi, "set_operator: NULL ctx or gauge");
+    QCD_REQUIRE(parity == 0 || parity == 1 || parity == 2, "set_operator: parity must be 0|1|2");
+    if (c_hi) {
+        QCD_REQUIRE(c_hi->precision == g_hi->precision && c_hi->geo.V == g_hi->geo.V, "set_operator: c_hi does not match g_hi");
+        QCD_REQUIRE(c_hi->kappa == kappa && c_hi->csw == csw, "set_operator: kappa/csw differ from the clover's");
+    }
+    if (g_lo) {
+        QCD_REQUIRE(g_lo->geo.V == g_hi->geo.V && g_lo->tb == g_hi->tb, "set_operator: g_lo does not match g_hi");
+        QCD_REQUIRE((c_lo != nullptr) == (c_hi != nullptr), "set_operator: c_lo and c_hi must both be given or both NULL");
+        if (c_lo) {
+            QCD_REQUIRE(c_lo->precision == g_lo->precision && c_lo->geo.V == g_lo->geo.V, "set_operator: c_lo does not match g_lo");
+            QCD_REQUIRE(c_lo->kappa == kappa && c_lo->csw == csw, "set_operator: kappa/csw differ from c_lo's");
+        }
+        QCD_REQUIRE(delta > 0.0 && delta < 1.0, "set_operator: delta must be in (0,1)");
+    }
+    ctx->g_hi = g_hi; ctx->g_lo = g_lo; ctx->c_hi = c_hi; ctx->c_lo = g_lo ? c_lo : nullptr;
+    ctx->kappa = kappa; ctx->csw = csw; ctx->op_parity = parity; ctx->delta = delta;
+    ctx->op_set = 1;
+    g_last_ctx = ctx;
+    return QCD_OK;
+}
+
+int qcd_apply_operator(qcd_ctx* ctx, void* out, const void* in, int flags)
+{
+    QCD_REQUIRE(ctx && ctx->op_set, "apply_operator: no operator set");
+    return qcd_dslash_ex(out, in, ctx->g_hi, ctx->c_hi, ctx->kappa, ctx->csw, ctx->op_parity, flags, nullptr);
+}
+
+int qcd_cg_solve_ex(qcd_ctx* ctx, void* x, const void* b, double tol, int maxiter, qcd_stats* stats)
+{
+    QCD_REQUIRE(ctx && ctx->op_set, "cg_solve: no operator set (qcd_set_operator)");
+    QCD_REQUIRE(x && b && (((uintptr_t)x | (uintptr_t)b) & 15u) == 0, "cg_solve: x/b must be non-NULL, 16-byte aligned");
+    QCD_REQUIRE(x != b, "cg_solve: x and b alias");
+    QCD_REQUIRE(tol > 0.0 && maxiter >= 0, "cg_solve: tol must be > 0 and maxiter >= 0");
+    qcd_stats st;
+    memset(&st, 0, sizeof(st));
+    cudaEvent_t e0, e1;
+    QCD_CHECK_CUDA(cudaEventCreate(&e0));
+    QCD_CHECK_CUDA(cudaEventCreate(&e1));
+    QCD_CHECK_CUDA(cudaEventRecord(e0, ctx->stream));
+    const int rc = ctx->g_lo ? cg_mixed(ctx, x, b, tol, maxiter, &st) : cg_pure(ctx, x, b, tol, maxiter, &st);
+    cudaEventRecord(e1, ctx->stream);
+    cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    st.seconds = ms * 1e-3;
+    {
+        const Op o = make_op(ctx, ctx->g_lo ? ctx->g_lo : ctx->g_hi, ctx->g_lo ? ctx->c_lo : ctx->c_hi);
+        st.flops = 2.0 * hop_flops_per_apply_M(o) * st.iters;
+        const double w = o.g->precision;
+        const double Vh = (double)o.g->geo.Vh;
+        const double hop_bytes = (48.0 + 8.0 * o.g->reconstruct) * w * Vh;
+        double per_M = 2.0 * hop_bytes + 24.0 * w * Vh + (o.c ? 2.0 * 72.0 * w * Vh : 0.0);
+        const double blas = (2.0 + 6.0 + 3.0) * w * (double)o.nreal; /* redot + cg_update + xpay */
+        st.bytes = (2.0 * per_M + blas) * st.iters;
+    }
+    if (stats) *stats = st;
+    return rc;
+}
+
+int qcd_cg_solve(void* x, const void* b, double tol, int maxiter)
+{
+    QCD_REQUIRE(g_last_ctx, "cg_solve: qcd_set_operator has not been called");
+    return qcd_cg_solve_ex(g_last_ctx, x, b, tol, maxiter, nullptr);
+}
+
+int qcd_cheb_apply(qcd_ctx* ctx, void* y, const void* v, const qcd_gauge* g, double kappa, const double* coeff, int degree, double scale)
+{
+    QCD_REQUIRE(ctx && g && y && v && coeff, "cheb_apply: NULL argument");
+    QCD_REQUIRE(degree >= 0 && scale > 0.0, "cheb_apply: degree must be >= 0 and scale > 0");
+    QCD_REQUIRE(y != v, "cheb_apply: y and v alias");
+    const int P = g->precision;
+    const size_t blk = (size_t)g->geo.Vh * 24 * P, full = 2 * blk, nreal = (size_t)g->geo.V * 24;
+    QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= 2 * full, "cheb_apply: workspace too small (need %zu bytes)", 2 * full);
+    char* ta = (char*)ctx->ws;
+    char* tb = ta + full;
+    if (degree == 0) {
+        RC(blas_copy(ctx, y, v, full));
+        return blas_axpby(ctx, host_scalar(0.0), v, host_scalar(coeff[0]), y, nreal, P);
+    }
+    RC(blas_copy(ctx, tb, v, full)); /* T_0 */
+    char* tk = tb;  /* T_k     */
+    char* tkm = ta; /* T_{k-1}, overwritten by T_{k+1} */
+    for (int k = 0; k < degree; k++) {
+        for (int p = 0; p < 2; p++) {
+            HopLaunch L;
+            memset(&L, 0, sizeof(L));
+            L.mode = HOP_CHEB;
+            L.in = tk + (1 - p) * blk;
+            L.z = tk + p * blk;
+            L.tm = tkm + p * blk;
+            L.y = (char*)y + p * blk;
+            L.b = -kappa;
+            L.c1 = (k == 0 ? 1.0 : 2.0) / scale;
+            L.c2 = (k == 0 ? 0.0 : -1.0);
+            L.ck = coeff[k + 1];
+            L.y_init = (k == 0);
+            L.c0 = coeff[0];
+            L.out_parity = p;
+            L.dagger = 0;
+            RC(hop_launch(ctx, g, L));
+        }
+        char* s = tk; tk = tkm; tkm = s;
+    }
+    return QCD_OK;
+}
+
+} /* extern "C" */
