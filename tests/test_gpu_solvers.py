@@ -1,0 +1,182 @@
+"""GPU parity: fused BLAS, CG on M^dag M, reliable-update mixed CG and the Chebyshev
+driver against the CPU oracle (same algorithm, same seeded inputs).  Criteria from
+BASELINE.json north_star: iteration count within +-2, true residual below tol."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as orc
+from paper_2001_05706_b200 import inputs
+
+from gpu_util import TOL, blocks, ctx, pack, parity_mask, relerr, to_dev, unpack
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("precision", [4, 8])
+@pytest.mark.parametrize("n", [4, 24 * 128, 24 * 1000 + 4, 24 * 8 * 8 * 8 * 16])
+def test_blas_matches_numpy_fp64(n, precision):
+    c = ctx()
+    rng = np.random.default_rng(n)
+    dt = {4: np.float32, 8: np.float64}[precision]
+    x, y, p, q = (rng.standard_normal(n).astype(dt) for _ in range(4))
+    X64, Y64, P64, Q64 = (v.astype(np.float64) for v in (x, y, p, q))
+    dx, dy, dp, dq = (torch.from_numpy(v).cuda() for v in (x, y, p, q))
+    tol = TOL[precision]
+    assert abs(c.norm2(dx) - np.dot(X64, X64)) <= 1e-13 * np.dot(X64, X64)
+    assert abs(c.redot(dx, dy) - np.dot(X64, Y64)) <= 1e-13 * np.sqrt(np.dot(X64, X64) * np.dot(Y64, Y64))
+    # deterministic: same bits every time
+    assert c.norm2(dx) == c.norm2(dx)
+    a, b = 0.37, -1.21
+    t = dy.clone(); c.axpy(a, dx, t)
+    assert relerr(t.cpu().numpy(), Y64 + a * X64) <= tol
+    t = dy.clone(); c.xpay(dx, a, t)
+    assert relerr(t.cpu().numpy(), X64 + a * Y64) <= tol
+    t = dy.clone(); c.axpby(a, dx, b, t)
+    assert relerr(t.cpu().numpy(), a * X64 + b * Y64) <= tol
+    tx, tr = dx.clone(), dy.clone()
+    r2 = c.cg_update(a, dp, dq, tx, tr)
+    want_r = Y64 - a * Q64
+    assert relerr(tx.cpu().numpy(), X64 + a * P64) <= tol
+    assert relerr(tr.cpu().numpy(), want_r) <= tol
+    got_r = tr.cpu().numpy().astype(np.float64)
+    assert abs(r2 - np.dot(got_r, got_r)) <= 1e-13 * r2
+
+
+def setup_operator(c, dims, kappa, csw, precision, recon, eps=0.5):
+    U = inputs.gauge_field(dims, eps, 0)
+    if precision == 4:
+        U = inputs.round_to_f32(U)
+    g = c.gauge_load(to_dev(U, precision), dims, precision, recon, -1)
+    A = Ainv = cl = None
+    if csw:
+        cl = c.clover_build(g, kappa, csw, precision)
+        F = orc.field_strength(U, dims)
+        A = orc.clover_matrix(F, dims, kappa * csw)
+        Ainv = orc.invert_12(A)
+    return U, g, cl, A, Ainv
+
+
+@pytest.mark.parametrize("mode", [2, 0])
+@pytest.mark.parametrize("csw", [0.0, 1.0])
+def test_cg_fp64_matches_oracle(mode, csw):
+    """configs[2] at a size the oracle finishes in seconds (8^3 x 16; same eps, kappa, csw, tol)."""
+    c = ctx()
+    dims, kappa, tol = (8, 8, 8, 16), 0.135, 1e-10
+    U, g, cl, A, Ainv = setup_operator(c, dims, kappa, csw, 8, 18)
+    b = inputs.spinor_field(dims, 0, 1)
+    if mode != 2:
+        b = b * (parity_mask(dims) == mode)
+    x_ref, st_ref = orc.cg(b, U, dims, kappa, tol, 5000, A, Ainv, -1, mode)
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    c.set_operator(g, None, cl, None, kappa, csw, mode)
+    pb = pack(c, b, dims, 8)
+    if mode == 2:
+        x = torch.empty_like(pb)
+        rc, st = c.cg_solve(x, pb, tol, 5000)
+        got = unpack(c, x, dims)
+    else:
+        full = torch.zeros_like(pb)
+        rc, st = c.cg_solve(blocks(full)[mode], blocks(pb)[mode], tol, 5000)
+        got = unpack(c, full, dims)
+    assert rc == 0 and st.converged == 1
+    assert abs(st.iters - st_ref["iters"]) <= 2
+    assert st.r_true < tol * 1.5 and st.r_iter <= tol
+    assert relerr(got, x_ref) <= 1e-8   # both solve N x = b to 1e-10 relative residual; cond(N) ~ 1e2
+
+
+def test_cg_reports_noconv_and_keeps_iterate():
+    c = ctx()
+    dims, kappa = (4, 4, 4, 8), 0.135
+    U, g, cl, A, Ainv = setup_operator(c, dims, kappa, 0.0, 8, 18)
+    b = inputs.spinor_field(dims, 0, 1)
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    c.set_operator(g, None, None, None, kappa, 0.0, 2)
+    pb = pack(c, b, dims, 8)
+    x = torch.empty_like(pb)
+    rc, st = c.cg_solve(x, pb, 1e-10, 7)
+    assert rc == 1 and st.iters == 7 and st.converged == 0
+    x_ref, st_ref = orc.cg(b, U, dims, kappa, 1e-10, 7)
+    assert relerr(unpack(c, x, dims), x_ref) <= 1e-11
+    assert abs(st.r_true - st_ref["r_true"]) <= 1e-9 * st_ref["r_true"]
+
+
+def test_cg_zero_source_and_plane_wave():
+    """b = 0 -> x = 0 in 0 iterations; free-field plane wave (pin P2) -> 1 iteration."""
+    c = ctx()
+    dims, kappa = (4, 4, 4, 4), 0.125
+    U = inputs.unit_gauge_field(dims)
+    g = c.gauge_load(to_dev(U, 8), dims, 8, 12, -1)
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    c.set_operator(g, None, None, None, kappa, 0.0, 2)
+    zero = torch.zeros(4 ** 4 * 24, dtype=torch.float64, device="cuda")
+    x = torch.ones_like(zero)
+    rc, st = c.cg_solve(x, zero, 1e-10, 100)
+    assert rc == 0 and st.iters == 0 and float(x.abs().max()) == 0.0
+    X, Y, Z, T = dims
+    n = (1, 0, 3, 2)
+    t, z, y, xx = np.meshgrid(np.arange(T), np.arange(Z), np.arange(Y), np.arange(X), indexing="ij")
+    ph = 2 * np.pi * (n[0] * xx / X + n[1] * y / Y + n[2] * z / Z + (n[3] + 0.5) * t / T)
+    u = np.random.default_rng(5).standard_normal((4, 3, 2))
+    uc = u[..., 0] + 1j * u[..., 1]
+    psi = np.exp(1j * ph)[..., None, None] * uc
+    b = np.stack([psi.real, psi.imag], axis=-1)
+    pb = pack(c, b, dims, 8)
+    rc, st = c.cg_solve(x, pb, 1e-10, 100)
+    assert rc == 0 and st.iters == 1
+    lam = 1.0151650429449555  # SURVEY.md Appendix A.5 (same n, kappa, dims)
+    assert relerr(unpack(c, x, dims), b / lam) <= 1e-12
+
+
+@pytest.mark.parametrize("mode", [2, 0])
+def test_mixed_cg_matches_oracle(mode):
+    """configs[3] at 8^3 x 16: fp32 12-real inner, fp64 18-real outer, delta = 0.1."""
+    c = ctx()
+    dims, kappa, csw, tol = (8, 8, 8, 16), 0.1355, 1.0, 1e-10
+    U, g_hi, c_hi, A, Ainv = setup_operator(c, dims, kappa, csw, 8, 18)
+    g_lo = c.gauge_load(to_dev(U, 8), dims, 4, 12, -1)       # fp64 links rounded to fp32 (S15)
+    c_lo = c.clover_build(g_hi, kappa, csw, 4)               # fp64 clover rounded to fp32 (S15)
+    b = inputs.spinor_field(dims, 0, 1)
+    if mode != 2:
+        b = b * (parity_mask(dims) == mode)
+    y_ref, st_ref = orc.cg_mixed(b, U, dims, kappa, tol, 5000, A, Ainv, -1, mode, 0.1)
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    c.set_operator(g_hi, g_lo, c_hi, c_lo, kappa, csw, mode, 0.1)
+    pb = pack(c, b, dims, 8)
+    if mode == 2:
+        y = torch.empty_like(pb)
+        rc, st = c.cg_solve(y, pb, tol, 5000)
+        got = unpack(c, y, dims)
+    else:
+        full = torch.zeros_like(pb)
+        rc, st = c.cg_solve(blocks(full)[mode], blocks(pb)[mode], tol, 5000)
+        got = unpack(c, full, dims)
+    assert rc == 0 and st.converged == 1
+    assert abs(st.iters - st_ref["iters"]) <= 2
+    assert abs(st.reliable_updates - st_ref["reliable_updates"]) <= 1
+    assert st.r_true < tol * 1.5
+    assert relerr(got, y_ref) <= 1e-8
+
+
+@pytest.mark.parametrize("precision,recon", [(4, 12), (8, 18)])
+def test_chebyshev_matches_oracle(precision, recon):
+    """configs[4] at 8^3 x 16: degree 100, kappa 0.2, scale 2.6, several vectors."""
+    c = ctx()
+    dims, kappa, scale = (8, 8, 8, 16), 0.2, 2.6
+    U, g, _, _, _ = setup_operator(c, dims, kappa, 0.0, precision, recon)
+    coeff = inputs.chebyshev_sign_coefficients(100)
+    c.ensure_workspace(c.workspace_bytes(dims, precision))
+    for i in range(3):
+        v = inputs.spinor_field(dims, 0, 10 + i)
+        if precision == 4:
+            v = inputs.round_to_f32(v)
+        want = orc.cheb(v, U, dims, kappa, coeff, scale)
+        pv = pack(c, v, dims, precision)
+        y = torch.empty_like(pv)
+        c.cheb_apply(y, pv, g, kappa, coeff, scale)
+        assert relerr(unpack(c, y, dims), want) <= TOL[precision]
+    # low degrees by the same path
+    for deg in (0, 1, 2):
+        want = orc.cheb(v, U, dims, kappa, coeff[:deg + 1], scale)
+        c.cheb_apply(y, pv, g, kappa, coeff[:deg + 1], scale)
+        assert relerr(unpack(c, y, dims), want) <= TOL[precision]
