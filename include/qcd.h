@@ -113,9 +113,11 @@ int qcd_spinor_pack(qcd_ctx* ctx, void* internal, const void* boundary, const in
                     int precision);
 int qcd_spinor_unpack(qcd_ctx* ctx, void* boundary, const void* internal, const int dims[4],
                       int precision);
-/* precision conversion of an internal-layout array of n reals (n multiple of 4) */
+/* precision conversion of internal-layout spinor blocks: nblocks = 1 (one parity) or 2
+ * (full field).  Layout-aware: a 128-bit chunk holds 2 complex in fp32 and 1 in fp64, so
+ * fp32 chunk c of site cb maps to the fp64 chunks 2c, 2c+1 of that site. */
 int qcd_convert(qcd_ctx* ctx, void* dst, int precision_dst, const void* src, int precision_src,
-                size_t nreal);
+                const int dims[4], int nblocks);
 
 /* ---- the stencil (north_star formula) --------------------------
  * qcd_hop: raw single-parity hopping term, the kernel the 1320 flop/site figure is

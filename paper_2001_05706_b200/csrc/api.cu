@@ -190,11 +190,15 @@ int qcd_spinor_unpack(qcd_ctx* ctx, void* boundary, const void* internal, const 
     return pack_common(ctx, const_cast<void*>(internal), boundary, dims, precision, 1);
 }
 
-int qcd_convert(qcd_ctx* ctx, void* dst, int pd, const void* src, int ps, size_t nreal)
+int qcd_convert(qcd_ctx* ctx, void* dst, int pd, const void* src, int ps, const int dims[4], int nblocks)
 {
     QCD_REQUIRE(ctx && aligned16(dst) && aligned16(src), "convert: bad pointer");
     QCD_REQUIRE((pd == 4 || pd == 8) && (ps == 4 || ps == 8), "convert: precision must be 4|8");
-    return blas_convert(ctx, dst, pd, src, ps, nreal);
+    QCD_REQUIRE(nblocks == 1 || nblocks == 2, "convert: nblocks must be 1 (one parity) or 2 (full field)");
+    Geom g;
+    int rc = make_geom(dims, &g);
+    if (rc) return rc;
+    return blas_convert(ctx, dst, pd, src, ps, (size_t)nblocks * g.Vh * 24, (size_t)g.Vh);
 }
 
 /* ---- workspace ------------------------------------------------------------------------ */

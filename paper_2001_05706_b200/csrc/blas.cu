@@ -123,24 +123,35 @@ __global__ void __launch_bounds__(BLAS_THREADS) cg_update_kernel(DevScalar a, co
     }
 }
 
+/* Mixed-precision kernels.  The internal spinor layout is [chunk][cb] with 128-bit
+ * chunks, so one fp32 chunk c (2 complex) of site cb corresponds to the fp64 chunks 2c
+ * and 2c+1 of the same site: float4 index (blk*6 + c)*Vh + cb  <->  double2 indices
+ * (blk*12 + 2c)*Vh + cb and (blk*12 + 2c + 1)*Vh + cb.  Both sides stay coalesced. */
+__device__ __forceinline__ size_t hi_index(size_t i, size_t Vh)
+{
+    const size_t plane = i / Vh, cb = i - plane * Vh; /* plane = blk*6 + c */
+    return 2 * plane * Vh + cb;
+}
+
 /* y_hi += x_lo ; x_lo = 0   (reliable update, reading O7) */
-__global__ void __launch_bounds__(BLAS_THREADS) accumulate_hi_kernel(double* y, float* x, size_t n4)
+__global__ void __launch_bounds__(BLAS_THREADS) accumulate_hi_kernel(double* y, float* x, size_t n4, size_t Vh)
 {
     float4* xv = reinterpret_cast<float4*>(x);
     double2* yv = reinterpret_cast<double2*>(y);
     for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < n4; i += (size_t)gridDim.x * BLAS_THREADS) {
         const float4 v = xv[i];
-        double2 a = yv[2 * i], b = yv[2 * i + 1];
+        const size_t j = hi_index(i, Vh);
+        double2 a = yv[j], b = yv[j + Vh];
         a.x += (double)v.x; a.y += (double)v.y; b.x += (double)v.z; b.y += (double)v.w;
-        yv[2 * i] = a;
-        yv[2 * i + 1] = b;
+        yv[j] = a;
+        yv[j + Vh] = b;
         xv[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
 }
 
 /* r_hi = b - t ; r_lo = (float) r_hi ; out = |r_hi|^2 */
-__global__ void __launch_bounds__(BLAS_THREADS) residual_hi_kernel(double* rh, float* rl, const double* b, const double* t, size_t n4, double* partial,
-                                   unsigned int* ticket, double* out)
+__global__ void __launch_bounds__(BLAS_THREADS) residual_hi_kernel(double* rh, float* rl, const double* b, const double* t, size_t n4, size_t Vh,
+                                   double* partial, unsigned int* ticket, double* out)
 {
     double s = 0.0;
     const double2* bv = reinterpret_cast<const double2*>(b);
@@ -148,20 +159,34 @@ __global__ void __launch_bounds__(BLAS_THREADS) residual_hi_kernel(double* rh, f
     double2* rv = reinterpret_cast<double2*>(rh);
     float4* lv = reinterpret_cast<float4*>(rl);
     for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < n4; i += (size_t)gridDim.x * BLAS_THREADS) {
-        const double2 b0 = bv[2 * i], b1 = bv[2 * i + 1], t0 = tv[2 * i], t1 = tv[2 * i + 1];
+        const size_t j = hi_index(i, Vh);
+        const double2 b0 = bv[j], b1 = bv[j + Vh], t0 = tv[j], t1 = tv[j + Vh];
         const double2 r0 = make_double2(b0.x - t0.x, b0.y - t0.y), r1 = make_double2(b1.x - t1.x, b1.y - t1.y);
         s += r0.x * r0.x + r0.y * r0.y + r1.x * r1.x + r1.y * r1.y;
-        rv[2 * i] = r0;
-        rv[2 * i + 1] = r1;
-        if (rl) lv[i] = make_float4((float)r0.x, (float)r0.y, (float)r1.x, (float)r1.y);
+        rv[j] = r0;
+        rv[j + Vh] = r1;
+        lv[i] = make_float4((float)r0.x, (float)r0.y, (float)r1.x, (float)r1.y);
     }
     double tot;
     if (grid_sum(s, partial, ticket, &tot)) *out = tot;
 }
 
-template <typename D, typename S> __global__ void __launch_bounds__(BLAS_THREADS) convert_kernel(D* dst, const S* src, size_t n)
+/* HI_TO_LO: lo = (float) hi ; else hi = (double) lo */
+template <int HI_TO_LO> __global__ void __launch_bounds__(BLAS_THREADS) convert_kernel(double* hi, float* lo, size_t n4, size_t Vh)
 {
-    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < n; i += (size_t)gridDim.x * BLAS_THREADS) dst[i] = (D)src[i];
+    float4* lv = reinterpret_cast<float4*>(lo);
+    double2* hv = reinterpret_cast<double2*>(hi);
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < n4; i += (size_t)gridDim.x * BLAS_THREADS) {
+        const size_t j = hi_index(i, Vh);
+        if (HI_TO_LO) {
+            const double2 a = hv[j], b = hv[j + Vh];
+            lv[i] = make_float4((float)a.x, (float)a.y, (float)b.x, (float)b.y);
+        } else {
+            const float4 v = lv[i];
+            hv[j] = make_double2((double)v.x, (double)v.y);
+            hv[j + Vh] = make_double2((double)v.z, (double)v.w);
+        }
+    }
 }
 
 int grid_for(const qcd_ctx* ctx, size_t nvec)
@@ -234,32 +259,30 @@ int blas_cg_update(qcd_ctx* ctx, DevScalar a, const void* p, const void* q, void
     return check_launch(ctx, "cg_update");
 }
 
-int blas_accumulate_hi(qcd_ctx* ctx, void* y_hi, void* x_lo, size_t nreal)
+int blas_accumulate_hi(qcd_ctx* ctx, void* y_hi, void* x_lo, size_t nreal, size_t Vh)
 {
     const size_t n4 = nreal / 4;
-    accumulate_hi_kernel<<<grid_for(ctx, n4), BLAS_THREADS, 0, ctx->stream>>>((double*)y_hi, (float*)x_lo, n4);
+    accumulate_hi_kernel<<<grid_for(ctx, n4), BLAS_THREADS, 0, ctx->stream>>>((double*)y_hi, (float*)x_lo, n4, Vh);
     return check_launch(ctx, "accumulate_hi");
 }
 
-int blas_residual_hi(qcd_ctx* ctx, void* r_hi, void* r_lo, const void* b, const void* t, size_t nreal, double* d_out)
+int blas_residual_hi(qcd_ctx* ctx, void* r_hi, void* r_lo, const void* b, const void* t, size_t nreal, size_t Vh, double* d_out)
 {
     const size_t n4 = nreal / 4;
-    residual_hi_kernel<<<grid_for(ctx, n4), BLAS_THREADS, 0, ctx->stream>>>((double*)r_hi, (float*)r_lo, (const double*)b, (const double*)t, n4,
+    residual_hi_kernel<<<grid_for(ctx, n4), BLAS_THREADS, 0, ctx->stream>>>((double*)r_hi, (float*)r_lo, (const double*)b, (const double*)t, n4, Vh,
                                                                           ctx->d_partial, ctx->d_ticket, d_out);
     return check_launch(ctx, "residual_hi");
 }
 
-int blas_convert(qcd_ctx* ctx, void* dst, int pdst, const void* src, int psrc, size_t nreal)
+int blas_convert(qcd_ctx* ctx, void* dst, int pdst, const void* src, int psrc, size_t nreal, size_t Vh)
 {
-    const int g = grid_for(ctx, nreal);
-    if (pdst == 4 && psrc == 8)
-        convert_kernel<float, double><<<g, BLAS_THREADS, 0, ctx->stream>>>((float*)dst, (const double*)src, nreal);
-    else if (pdst == 8 && psrc == 4)
-        convert_kernel<double, float><<<g, BLAS_THREADS, 0, ctx->stream>>>((double*)dst, (const float*)src, nreal);
-    else if (pdst == 4 && psrc == 4)
-        convert_kernel<float, float><<<g, BLAS_THREADS, 0, ctx->stream>>>((float*)dst, (const float*)src, nreal);
+    if (pdst == psrc) return blas_copy(ctx, dst, src, nreal * (size_t)pdst);
+    const size_t n4 = nreal / 4;
+    const int g = grid_for(ctx, n4);
+    if (pdst == 4)
+        convert_kernel<1><<<g, BLAS_THREADS, 0, ctx->stream>>>((double*)const_cast<void*>(src), (float*)dst, n4, Vh);
     else
-        convert_kernel<double, double><<<g, BLAS_THREADS, 0, ctx->stream>>>((double*)dst, (const double*)src, nreal);
+        convert_kernel<0><<<g, BLAS_THREADS, 0, ctx->stream>>>((double*)dst, (float*)const_cast<void*>(src), n4, Vh);
     return check_launch(ctx, "convert");
 }
 

@@ -134,11 +134,12 @@ int blas_redot(qcd_ctx*, const void* x, const void* y, size_t nreal, int prec, d
 int blas_cg_update(qcd_ctx*, DevScalar a, const void* p, const void* q, void* x, void* r,
                    size_t nreal, int prec, double* d_out, double* d_beta, const double* d_rho_old);
 /* y(hi) += x(lo); x = 0 */
-int blas_accumulate_hi(qcd_ctx*, void* y_hi, void* x_lo, size_t nreal);
+int blas_accumulate_hi(qcd_ctx*, void* y_hi, void* x_lo, size_t nreal, size_t Vh);
 /* r_hi = b - t (fp64); r_lo = (float) r_hi; *d_out = |r_hi|^2 */
 int blas_residual_hi(qcd_ctx*, void* r_hi, void* r_lo, const void* b, const void* t, size_t nreal,
-                     double* d_out);
-int blas_convert(qcd_ctx*, void* dst, int pdst, const void* src, int psrc, size_t nreal);
+                     size_t Vh, double* d_out);
+/* internal-layout spinor blocks of Vh sites each (nreal = nblocks*24*Vh), layout-aware */
+int blas_convert(qcd_ctx*, void* dst, int pdst, const void* src, int psrc, size_t nreal, size_t Vh);
 int blas_zero(qcd_ctx*, void* x, size_t bytes);
 int blas_copy(qcd_ctx*, void* dst, const void* src, size_t bytes);
 

@@ -8,6 +8,8 @@
  * doubles per iteration for the stopping test.
  */
 #include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "qcd_internal.h"
@@ -135,12 +137,12 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
     void *x = wl, *r = wl + ol.bytes, *p = wl + 2 * ol.bytes, *q = wl + 3 * ol.bytes, *tl = wl + 4 * ol.bytes, *l2 = wl + 5 * ol.bytes;
     double* d = ctx->d_scalar;
     double* h = ctx->h_scalar;
-    const size_t n = oh.nreal;
+    const size_t n = oh.nreal, Vh = (size_t)oh.g->geo.Vh;
 
     RC(set_one(ctx));
     RC(blas_zero(ctx, y, oh.bytes));
     RC(blas_zero(ctx, x, ol.bytes));
-    RC(blas_convert(ctx, r, 4, b, 8, n));
+    RC(blas_convert(ctx, r, 4, b, 8, n, Vh));
     RC(blas_copy(ctx, p, r, ol.bytes));
     int cur = S_RHO_A, nxt = S_RHO_B;
     RC(blas_norm2(ctx, b, n, 8, d + S_AUX));
@@ -150,6 +152,7 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
     double rho = h[cur];
     double rmax = sqrt(rho), rhnorm = bnorm;
     int k = 0, conv = (bnorm == 0.0), brk = 0, nup = 0;
+    const bool trace = getenv("QCD_TRACE") != nullptr;
     while (!conv && k < maxiter) {
         k++;
         RC(apply_N(ol, q, p, tl, l2));
@@ -159,16 +162,18 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
         if (!(h[S_PQ] > 0.0)) { brk = 1; break; }
         double rho2 = h[nxt];
         const double rnorm = sqrt(rho2);
+        if (trace) fprintf(stderr, "mixed k=%d rho=%.6e pq=%.6e rho2=%.6e rmax=%.3e\n", k, rho, h[S_PQ], rho2, rmax);
         if (rnorm > rmax) rmax = rnorm;
         if (rnorm < ctx->delta * rmax || rnorm <= tol * bnorm) {
-            RC(blas_accumulate_hi(ctx, y, x, n));                 /* y += x ; x = 0          */
+            RC(blas_accumulate_hi(ctx, y, x, n, Vh));                 /* y += x ; x = 0          */
             RC(apply_N(oh, th, y, h1, h2));                       /* th = N_hi y             */
-            RC(blas_residual_hi(ctx, rh, r, b, th, n, d + nxt));  /* rh = b - th ; r = (f)rh */
+            RC(blas_residual_hi(ctx, rh, r, b, th, n, Vh, d + nxt));  /* rh = b - th ; r = (f)rh */
             RC(fetch(ctx, nxt, 1));
             rho2 = h[nxt];
             rhnorm = sqrt(rho2);
             rmax = rhnorm;
             nup++;
+            if (trace) fprintf(stderr, "mixed   reliable update %d: |r_hi|/|b| = %.6e\n", nup, rhnorm / bnorm);
             if (rhnorm <= tol * bnorm) { conv = 1; break; }
         }
         const float beta = (float)(rho2 / rho);
@@ -176,7 +181,7 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
         rho = rho2;
         const int s = cur; cur = nxt; nxt = s;
     }
-    if (!conv) RC(blas_accumulate_hi(ctx, y, x, n));
+    if (!conv) RC(blas_accumulate_hi(ctx, y, x, n, Vh));
     double r_true = 0.0;
     RC(true_residual(oh, y, b, th, h1, h2, bnorm, &r_true));
     if (st) {

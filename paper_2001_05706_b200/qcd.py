@@ -54,7 +54,7 @@ SIGNATURES = {
     "qcd_spinor_bytes": (_sz, [_dims_t, _i]),
     "qcd_spinor_pack": (_i, [_vp, _vp, _vp, _dims_t, _i]),
     "qcd_spinor_unpack": (_i, [_vp, _vp, _vp, _dims_t, _i]),
-    "qcd_convert": (_i, [_vp, _vp, _i, _vp, _i, _sz]),
+    "qcd_convert": (_i, [_vp, _vp, _i, _vp, _i, _dims_t, _i]),
     "qcd_hop": (_i, [_vp, _vp, _vp, _i, _i, _dims_t, _i]),
     "qcd_hop_xpay": (_i, [_vp, _vp, _vp, _d, _d, _vp, _i, _i]),
     "qcd_dslash": (_i, [_vp, _vp, _vp, _vp, _d, _d, _i, _dims_t, _i]),
@@ -195,9 +195,9 @@ class Context:
         _check(lib().qcd_spinor_unpack(self.h, _ptr(boundary), _ptr(internal), _dims(dims), _prec(internal)))
         return boundary
 
-    def convert(self, src: torch.Tensor, precision: int) -> torch.Tensor:
+    def convert(self, src: torch.Tensor, precision: int, dims, nblocks: int) -> torch.Tensor:
         dst = torch.empty(src.numel(), dtype=_dtype(precision), device=self.device)
-        _check(lib().qcd_convert(self.h, _ptr(dst), precision, _ptr(src), _prec(src), src.numel()))
+        _check(lib().qcd_convert(self.h, _ptr(dst), precision, _ptr(src), _prec(src), _dims(dims), nblocks))
         return dst
 
     # ---- stencil -------------------------------------------------------------------

@@ -169,3 +169,18 @@ def test_argument_errors_are_reported():
     out = torch.empty_like(pin)
     with pytest.raises(qcd.QcdError):
         c.dslash(out, pin, g, cl, 0.136, 1.0, 2)             # kappa differs from the clover's (S10)
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 2, 8)])
+def test_convert_is_layout_aware(dims):
+    """fp32 <-> fp64 conversion of internal fields keeps (site, spin, colour) in place."""
+    c = ctx()
+    psi = inputs.spinor_field(dims, 1, 0)
+    p64 = pack(c, psi, dims, 8)
+    p32 = c.convert(p64, 4, dims, 2)
+    assert torch.equal(c.spinor_unpack(p32, dims), to_dev(psi, 8).float())
+    back = c.convert(p32, 8, dims, 2)
+    assert torch.equal(c.spinor_unpack(back, dims), to_dev(psi, 8).float().double())
+    h = p64.numel() // 2
+    one = c.convert(p64[h:], 4, dims, 1)
+    assert torch.equal(one, p32[h:])
