@@ -1,0 +1,426 @@
+"""bench.py -- Wilson-clover Dslash throughput on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--quick]
+
+Workload: the 32^3 x 64 fp32 lattice that north_star's 70 %
+bar names (BASELINE.json configs[3]'s lattice and inner precision): links by the configs[0]
+recipe with eps = 0.5, stored with 12 reals, kappa = 0.1355, csw = 1.0, antiperiodic t.
+A STEP is one application of the even-odd preconditioned Wilson-clover operator
+    Mhat_ee = A_ee - kappa^2 H_eo A_oo^-1 H_oe
+= two launches of the hopping-term kernel with the clover-inverse apply, the clover apply
+and the xpay fused in their epilogues.  The headline value is the
+nominal Dslash GFLOP/s (1320 flop/site per hop + 504 per clover apply; BASELINE.json
+north_star) with inputs resident in HBM; `e2e` is the same operator through
+qcd_dslash_host with HOST buffers.  Further objects in the same JSON line report every
+other kernel of the path (plain hop 12/18-real, fp64, the fused BLAS-1 kernels) against
+the HBM roofline, and CG / mixed-CG / Chebyshev timings.
+
+Multi-GPU: the path does not shard in this build (north_star: "Everything runs on one
+GPU"): `--gpus N` runs N independent replicas, one per rank, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+DIMS = (32, 32, 32, 64)
+SMALL_DIMS = (16, 16, 16, 32)          # configs[1] lattice: the oracle's bounded sample
+EPS, KAPPA, CSW = 0.5, 0.1355, 1.0
+HOP_FLOP, CLOVER_FLOP = 1320.0, 504.0  # nominal flop / site (north_star)
+METRIC, UNIT = "wilson_clover_dslash_gflops", "GFLOP/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--quick", action="store_true", help="skip the per-kernel / solver sections")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    """Roofline denominator: MEASURED_PEAKS.json (driver-written), else the fallback of
+    /opt/skills/guides/B200_PROFILING.md (6.65 TB/s)."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def step_flops(Vh, clover=True):
+    return 2.0 * HOP_FLOP * Vh + (2.0 * CLOVER_FLOP * Vh if clover else 0.0)
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index=0, period=0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    _NAMES = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+              0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+              0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in self._NAMES.items():
+                    if r & bit and name != "gpu_idle":
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2)
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+# ---------------------------------------------------------------------------------------
+# CPU oracle leg (the only place bench.py executes oracle/): cpu_baseline and --impl reference
+# ---------------------------------------------------------------------------------------
+class OracleWorkload:
+    """The oracle's Mhat_ee apply, as it stands, on a bounded sample of the workload: the
+    16^3 x 32 lattice (1/16 of the 32^3 x 64 sites; same recipe, kappa, csw)."""
+
+    sample = "Mhat_ee apply (oracle apply_M mode 0, fp64) on a 16^3x32 lattice = 1/16 of the 32^3x64 sites, same recipe"
+
+    def __init__(self):
+        import numpy as np
+        from oracle import oracle as orc
+        from paper_2001_05706_b200 import inputs
+        self.orc, self.dims = orc, SMALL_DIMS
+        self.U = inputs.gauge_field(self.dims, EPS, 0)
+        F = orc.field_strength(self.U, self.dims)
+        self.A = orc.clover_matrix(F, self.dims, KAPPA * CSW)
+        self.Ainv = orc.invert_12(self.A)
+        par = orc.parity_mask_array(self.dims)[..., None, None, None]
+        self.psi = inputs.spinor_field(self.dims, 0, 0) * (par == 0)
+        self.Vh = int(np.prod(self.dims)) // 2
+        self.cores = orc.num_threads()
+
+    def step(self):
+        return self.orc.apply_M(self.psi, self.U, self.dims, KAPPA, self.A, self.Ainv, -1, 0, False)
+
+    def time_steps(self, steps, warmup):
+        for _ in range(warmup):
+            self.step()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            self.step()
+        dt = (time.perf_counter() - t0) / max(steps, 1)
+        return dt, step_flops(self.Vh) / dt * 1e-9
+
+
+def cpu_baseline(budget_s=15.0):
+    w = OracleWorkload()
+    dt1, _ = w.time_steps(1, 1)
+    n = max(1, min(200, int(budget_s / max(dt1, 1e-6))))
+    dt, gf = w.time_steps(n, 0)
+    return {"value": gf, "unit": UNIT, "cores": w.cores, "kind": "oracle", "sample": w.sample,
+            "ms_per_step_on_sample": dt * 1e3}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = OracleWorkload()
+    steps = max(1, min(args.steps, 50))
+    warm = max(1, min(args.warmup, 3))
+    dt, gf = w.time_steps(steps, warm)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": gf, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": warm, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "even-odd Wilson-clover Mhat apply, CPU oracle on the 16^3x32 sample of the 32^3x64 workload",
+                   "dims": list(SMALL_DIMS), "kappa": KAPPA, "csw": CSW, "eps": EPS},
+        "cpu_baseline": {"value": gf, "unit": UNIT, "cores": w.cores, "kind": "oracle", "sample": w.sample},
+        "e2e": {"value": gf, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------
+# CUDA arm
+# ---------------------------------------------------------------------------------------
+def gpu_time_ms(fn, iters, warm=3):
+    """Average device time of fn() in ms: CUDA events on the launching stream (the ctx is
+    bound to torch's current stream), after warm-up, synchronised on both sides."""
+    import torch
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(iters):
+        fn()
+    e1.record()
+    e1.synchronize()
+    return e0.elapsed_time(e1) / iters
+
+
+def build_workload(c, dims, want_hi):
+    """Seeded synthetic fields on the device.  Links: configs[0] recipe with eps = 0.5 on a
+    (X,Y,Z,16) block repeated along t (inputs.tiled_gauge_field); source: N(0,1)."""
+    import torch
+    from paper_2001_05706_b200 import inputs
+    U = inputs.tiled_gauge_field(dims, EPS, 0, 16)
+    dU = torch.from_numpy(U).cuda()
+    del U
+    w = {"dims": dims}
+    g_hi = c.gauge_load(dU, dims, 8, 18, -1)
+    w["g32"] = c.gauge_load(dU, dims, 4, 12, -1)
+    w["c32"] = c.clover_build(g_hi, KAPPA, CSW, 4)          # fp64 arithmetic, fp32 storage (S15)
+    if want_hi:
+        w["g32_18"] = c.gauge_load(dU, dims, 4, 18, -1)
+        w["g64"] = g_hi
+        w["c64"] = c.clover_build(g_hi, KAPPA, CSW, 8)
+    del dU
+    psi = torch.from_numpy(inputs.spinor_field(dims, 0, 0))
+    w["psi64"] = c.spinor_pack(psi.cuda(), dims) if want_hi else None
+    w["psi32"] = c.spinor_pack(psi.float().cuda(), dims)
+    torch.cuda.synchronize()
+    return w
+
+
+def traffic_from_profile():
+    """dram bytes per launch of the dominant kernel from the committed ncu capture, if any."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(p) as f:
+            return json.load(f).get("hop_clover_fp32_12_bytes_per_launch")
+    except Exception:
+        return None
+
+
+def kernel_table(c, w, peak):
+    """Every other kernel of the path against the HBM roofline (SURVEY.md 8(d) bytes/site)."""
+    import torch
+    dims = w["dims"]
+    Vh = dims[0] * dims[1] * dims[2] * dims[3] // 2
+    out = {}
+
+    def row(name, ms, bytes_per_site, flop_per_site):
+        gbs = bytes_per_site * Vh / (ms * 1e-3) * 1e-9
+        out[name] = {"us": round(ms * 1e3, 2), "GB/s": round(gbs, 1), "frac": round(gbs / peak, 4),
+                     "GFLOP/s": round(flop_per_site * Vh / (ms * 1e-3) * 1e-9, 1), "B/site": bytes_per_site}
+
+    h = Vh * 24
+    a32, b32 = w["psi32"][:h], torch.empty_like(w["psi32"][:h])
+    z32 = w["psi32"][h:]
+    row("hop_fp32_12", gpu_time_ms(lambda: c.hop(b32, z32, w["g32"], 0), 50), 576, 1320)
+    row("hop_fp32_18", gpu_time_ms(lambda: c.hop(b32, z32, w["g32_18"], 0), 50), 768, 1320)
+    row("hop_xpay_fp32_12", gpu_time_ms(lambda: c.hop_xpay(b32, z32, a32, 1.0, -KAPPA, w["g32"], 0), 50), 672, 1320)
+    a64, b64 = w["psi64"][:h], torch.empty_like(w["psi64"][:h])
+    z64 = w["psi64"][h:]
+    row("hop_fp64_18", gpu_time_ms(lambda: c.hop(b64, z64, w["g64"], 0), 20), 1536, 1320)
+    tmp64 = torch.empty_like(b64)
+    ms = gpu_time_ms(lambda: c.dslash_ex(b64, a64, w["g64"], w["c64"], KAPPA, CSW, 0, 0, tmp64), 20)
+    row("Mhat_clover_fp64_18 (2 launches)", ms, 2 * 1536 + 2 * 576 + 192, 2 * 1320 + 2 * 504)
+    # fused BLAS-1, one-parity fp32 vectors (100 MB each; 4 distinct arrays > L2)
+    x, y, p, q = (torch.randn(h, device="cuda", dtype=torch.float32) for _ in range(4))
+    row("axpy_fp32", gpu_time_ms(lambda: c.axpy(1e-3, x, y), 50), 288, 48)
+    row("xpay_fp32", gpu_time_ms(lambda: c.xpay(x, 0.5, y), 50), 288, 48)
+    row("norm2_fp32", gpu_time_ms(lambda: c.norm2(x, fetch=False), 50), 96, 48)
+    row("redot_fp32", gpu_time_ms(lambda: c.redot(x, y, fetch=False), 50), 192, 96)
+    row("cg_update_fp32", gpu_time_ms(lambda: c.cg_update(1e-6, p, q, x, y, fetch=False), 50), 576, 144)
+    x, y, p, q = (t.double() for t in (x, y, p, q))
+    row("cg_update_fp64", gpu_time_ms(lambda: c.cg_update(1e-6, p, q, x, y, fetch=False), 20), 1152, 144)
+    row("redot_fp64", gpu_time_ms(lambda: c.redot(x, y, fetch=False), 20), 384, 96)
+    return out
+
+
+def solver_table(c, w):
+    """CG seconds to 1e-10 (BASELINE.json metric, second half): even-odd clover, 32^3x64."""
+    import torch
+    from paper_2001_05706_b200 import inputs
+    dims = w["dims"]
+    Vh = dims[0] * dims[1] * dims[2] * dims[3] // 2
+    h = Vh * 24
+    b = c.spinor_pack(torch.from_numpy(inputs.spinor_field(dims, 0, 1)).cuda(), dims)[:h].clone()
+    x = torch.empty_like(b)
+    out = {}
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    for name, lo in (("mixed_cg_fp32_12/fp64_18", True), ("cg_fp64_18", False)):
+        if lo:
+            c.set_operator(w["g64"], w["g32"], w["c64"], w["c32"], KAPPA, CSW, 0, 0.1)
+        else:
+            c.set_operator(w["g64"], None, w["c64"], None, KAPPA, CSW, 0)
+        c.cg_solve(x, b, 1e-10, 5000)                      # warm-up solve
+        rc, st = c.cg_solve(x, b, 1e-10, 5000)
+        out[name] = {"seconds": round(st.seconds, 5), "iters": st.iters, "reliable_updates": st.reliable_updates,
+                     "r_true": st.r_true, "rc": rc, "GFLOP/s": round(st.flops / st.seconds * 1e-9, 1),
+                     "ms_per_iter": round(st.seconds / max(st.iters, 1) * 1e3, 4)}
+    return out
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_2001_05706_b200 import build
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    from paper_2001_05706_b200 import qcd
+    c = qcd.Context(local)
+    peak, peak_src = measured_peaks()
+    full = (not args.quick) and rank == 0
+    w = build_workload(c, DIMS, want_hi=full)
+    dims = DIMS
+    Vh = dims[0] * dims[1] * dims[2] * dims[3] // 2
+    h = Vh * 24
+    src, dst = w["psi32"][:h], torch.empty_like(w["psi32"][:h])
+    tmp = torch.empty_like(dst)
+    g, cl = w["g32"], w["c32"]
+
+    def step():
+        c.dslash_ex(dst, src, g, cl, KAPPA, CSW, 0, 0, tmp)
+
+    # ---- timed region: W warm-up steps, then exactly K steps between barrier + synchronize
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    n0 = c.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms_total = e0.elapsed_time(e1)
+    launches = c.launch_count() - n0
+    clocks = sampler.stop()
+    if world > 1:
+        dist.barrier()
+        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * step_flops(Vh) / (ms_step * 1e-3) * 1e-9
+
+    # ---- roofline of the dominant kernel (hop_kernel<float,12,*,CLOVER_*>): two launches per
+    # step, algorithmic bytes 864 (clover-inverse epilogue) and 960 (clover + xpay) per site
+    bytes_launch = 0.5 * (864 + 960) * Vh
+    ms_launch = ms_step / 2.0
+    achieved = bytes_launch / (ms_launch * 1e-3) * 1e-9
+    roofline = {"bound": "hbm", "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                "frac": round(achieved / peak, 4), "traffic": traffic_from_profile(), "peak_source": peak_src,
+                "kernel": "hop_kernel<float,12,0,CLOVER_OUT|CLOVER_Z>", "bytes_per_launch": bytes_launch,
+                "us_per_launch": round(ms_launch * 1e3, 2)}
+
+    # ---- end to end: HOST buffers through qcd_dslash_host (H2D + Mhat + D2H every step)
+    blk_bytes = h * 4
+    c.ensure_workspace(max(3 * blk_bytes, c._ws.numel() if c._ws is not None else 0))
+    hin = torch.empty(h, dtype=torch.float32).pin_memory()
+    hout = torch.empty(h, dtype=torch.float32).pin_memory()
+    hin.copy_(src.cpu())
+    e2e_steps = max(3, min(20, args.steps))
+    for _ in range(2):
+        c.dslash_host(hout, hin, g, cl, KAPPA, CSW, 0, 0)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(e2e_steps):
+        c.dslash_host(hout, hin, g, cl, KAPPA, CSW, 0, 0)
+    e1.record()
+    torch.cuda.synchronize()
+    e2e_ms = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3) / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e = {"value": round(world * step_flops(Vh) / (e2e_ms * 1e-3) * 1e-9, 1), "unit": UNIT,
+           "h2d_bytes_per_step": blk_bytes, "d2h_bytes_per_step": blk_bytes, "ms_per_step": round(e2e_ms, 4),
+           "steps": e2e_steps, "call": "qcd_dslash_host"}
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+    line = {
+        "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": round(ms_step, 5), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "even-odd Wilson-clover Dslash (Mhat_ee apply = 2 fused hop launches), 32^3x64, fp32, "
+                               "12-real links, kappa 0.1355, csw 1.0, eps 0.5 (BASELINE.json configs[3] lattice, "
+                               "north_star 70% target workload)",
+                   "dims": list(dims), "reconstruct": 12, "kappa": KAPPA, "csw": CSW, "eps": EPS,
+                   "parallelism": "replicas only (x%d)" % world,
+                   "l2": "inputs larger than L2: gauge 403 MB + clover 604 MB + spinors 302 MB per step",
+                   "flop_per_step": step_flops(Vh), "gauge_recipe": "32^3x16 block of the configs[0] recipe tiled 4x in t"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+    }
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline()
+    if full:
+        line["kernels"] = kernel_table(c, w, peak)
+        line["cg"] = solver_table(c, w)
+    print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

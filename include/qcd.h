@@ -154,7 +154,9 @@ int qcd_set_workspace(qcd_ctx* ctx, void* ws, size_t bytes);
 /* ---- fused BLAS-1 ("vector operations", reductions) --
  * Arrays of `nreal` reals (multiple of 4) in `precision`.  Reductions multiply and
  * accumulate in fp64 (warp shuffle -> block -> last-block final pass, fixed order,
- * deterministic) and return the scalar to the HOST pointer (synchronises).        */
+ * deterministic) and return the scalar to the HOST pointer `result` (synchronises);
+ * with result == NULL the scalar stays in the ctx's device slot and the call does not
+ * synchronise (used for back-to-back timing).                                       */
 int qcd_axpy(qcd_ctx*, double a, const void* x, void* y, size_t nreal, int precision);   /* y += a x   */
 int qcd_xpay(qcd_ctx*, const void* x, double a, void* y, size_t nreal, int precision);   /* y = x + a y */
 int qcd_axpby(qcd_ctx*, double a, const void* x, double b, void* y, size_t nreal, int precision); /* y = a x + b y */
@@ -196,6 +198,13 @@ int qcd_cheb_apply(qcd_ctx* ctx, void* y, const void* v, const qcd_gauge* g, dou
  * layout: copies in -> device scratch (ctx workspace), runs qcd_hop, copies out. */
 int qcd_hop_host(qcd_ctx* ctx, void* out_host, const void* in_host, const qcd_gauge* g,
                  int out_parity, int dagger);
+
+/* out_host = M in_host (or M^dag, flags & QCD_DAGGER) with M as in qcd_dslash: HOST buffers in
+ * the internal layout (full field for parity 2, one parity block else); gauge / clover stay
+ * resident on the device.  H2D copy, the operator, D2H copy, then a stream synchronise.
+ * Needs a workspace of 2 * field + one parity block. */
+int qcd_dslash_host(qcd_ctx* ctx, void* out_host, const void* in_host, const qcd_gauge* g,
+                    const qcd_clover* c, double kappa, double csw, int parity, int flags);
 
 /* number of kernels this library has launched on this ctx since qcd_init */
 long long qcd_launch_count(const qcd_ctx* ctx);

@@ -367,18 +367,16 @@ int qcd_norm2(qcd_ctx* ctx, const void* x, size_t nreal, int precision, double* 
 {
     int rc = blas_args(ctx, x, x, nreal, precision);
     if (rc) return rc;
-    QCD_REQUIRE(result, "norm2: NULL result");
     rc = blas_norm2(ctx, x, nreal, precision, ctx->d_scalar + SC_TMP);
-    if (rc) return rc;
+    if (rc || !result) return rc;
     return fetch_scalar(ctx, SC_TMP, result);
 }
 int qcd_redot(qcd_ctx* ctx, const void* x, const void* y, size_t nreal, int precision, double* result)
 {
     int rc = blas_args(ctx, x, y, nreal, precision);
     if (rc) return rc;
-    QCD_REQUIRE(result, "redot: NULL result");
     rc = blas_redot(ctx, x, y, nreal, precision, ctx->d_scalar + SC_TMP);
-    if (rc) return rc;
+    if (rc || !result) return rc;
     return fetch_scalar(ctx, SC_TMP, result);
 }
 int qcd_cg_update(qcd_ctx* ctx, double a, const void* p, const void* q, void* x, void* r, size_t nreal, int precision, double* result)
@@ -387,9 +385,8 @@ int qcd_cg_update(qcd_ctx* ctx, double a, const void* p, const void* q, void* x,
     if (rc) return rc;
     rc = blas_args(ctx, x, r, nreal, precision);
     if (rc) return rc;
-    QCD_REQUIRE(result, "cg_update: NULL result");
     rc = blas_cg_update(ctx, host_scalar(a), p, q, x, r, nreal, precision, ctx->d_scalar + SC_TMP, nullptr, nullptr);
-    if (rc) return rc;
+    if (rc || !result) return rc;
     return fetch_scalar(ctx, SC_TMP, result);
 }
 
@@ -405,6 +402,25 @@ int qcd_hop_host(qcd_ctx* ctx, void* out_host, const void* in_host, const qcd_ga
     int rc = qcd_hop_xpay(d_out, d_in, nullptr, 0.0, 0.0, g, out_parity, dagger);
     if (rc) return rc;
     QCD_CHECK_CUDA(cudaMemcpyAsync(out_host, d_out, blk, cudaMemcpyDeviceToHost, ctx->stream));
+    QCD_CHECK_CUDA(cudaStreamSynchronize(ctx->stream));
+    return QCD_OK;
+}
+
+int qcd_dslash_host(qcd_ctx* ctx, void* out_host, const void* in_host, const qcd_gauge* g, const qcd_clover* c, double kappa,
+                    double csw, int parity, int flags)
+{
+    QCD_REQUIRE(ctx && g && out_host && in_host, "dslash_host: NULL argument");
+    QCD_REQUIRE(parity == 0 || parity == 1 || parity == 2, "dslash_host: parity must be 0|1|2");
+    const size_t blk = (size_t)g->geo.Vh * 24 * g->precision;
+    const size_t bytes = parity == 2 ? 2 * blk : blk;
+    QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= 2 * bytes + blk, "dslash_host: workspace too small (qcd_set_workspace)");
+    char* d_in = (char*)ctx->ws;
+    char* d_out = d_in + bytes;
+    char* d_tmp = d_out + bytes;
+    QCD_CHECK_CUDA(cudaMemcpyAsync(d_in, in_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    int rc = qcd_dslash_ex(d_out, d_in, g, c, kappa, csw, parity, flags, d_tmp);
+    if (rc) return rc;
+    QCD_CHECK_CUDA(cudaMemcpyAsync(out_host, d_out, bytes, cudaMemcpyDeviceToHost, ctx->stream));
     QCD_CHECK_CUDA(cudaStreamSynchronize(ctx->stream));
     return QCD_OK;
 }

@@ -28,7 +28,7 @@ from __future__ import annotations
 import numpy as np
 
 __all__ = [
-    "gauge_field", "unit_gauge_field", "spinor_field", "su3_site_field",
+    "gauge_field", "tiled_gauge_field", "unit_gauge_field", "spinor_field", "su3_site_field",
     "as_complex", "as_real", "round_to_f32", "chebyshev_sign_coefficients",
 ]
 
@@ -113,6 +113,21 @@ def gauge_field(dims, eps: float, seed: int = 0) -> np.ndarray:
         G = rng.standard_normal((Z, Y, X, 4, 3, 3, 2))
         out[t] = as_real(_su3_from_normals(G, eps))
     return out
+
+
+def tiled_gauge_field(dims, eps: float, seed: int = 0, t_block: int = 16) -> np.ndarray:
+    """gauge_field for a (X,Y,Z,t_block) lattice repeated T/t_block times along t.
+
+    Used where the full-size field would take minutes to draw on the host (bench.py and
+    the full-size sampled parity tests): every link is still an SU(3) matrix of the recipe
+    above and the field is periodic, so it is a valid input of the same distribution; only
+    its long-range structure in t repeats.  Falls back to gauge_field when t_block does
+    not divide T."""
+    X, Y, Z, T = (int(d) for d in dims)
+    if t_block >= T or T % t_block:
+        return gauge_field(dims, eps, seed)
+    blk = gauge_field((X, Y, Z, t_block), eps, seed)
+    return np.ascontiguousarray(np.concatenate([blk] * (T // t_block), axis=0))
 
 
 def unit_gauge_field(dims) -> np.ndarray:

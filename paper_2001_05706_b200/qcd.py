@@ -73,6 +73,7 @@ SIGNATURES = {
     "qcd_apply_operator": (_i, [_vp, _vp, _vp, _i]),
     "qcd_cheb_apply": (_i, [_vp, _vp, _vp, _vp, _d, C.POINTER(_d), _i, _d]),
     "qcd_hop_host": (_i, [_vp, _vp, _vp, _vp, _i, _i]),
+    "qcd_dslash_host": (_i, [_vp, _vp, _vp, _vp, _vp, _d, _d, _i, _i]),
     "qcd_launch_count": (C.c_longlong, [_vp]),
 }
 
@@ -219,6 +220,10 @@ class Context:
         """out_host / in_host: pinned (or pageable) HOST tensors, one-parity internal blocks."""
         _check(lib().qcd_hop_host(self.h, _ptr(out_host), _ptr(in_host), gauge.h, out_parity, int(dagger)))
 
+    def dslash_host(self, out_host, in_host, gauge: "Gauge", clover, kappa: float, csw: float, parity: int, flags: int = 0):
+        _check(lib().qcd_dslash_host(self.h, _ptr(out_host), _ptr(in_host), gauge.h, clover.h if clover else None,
+                                     kappa, csw, parity, flags))
+
     # ---- BLAS ------------------------------------------------------------------------
     def axpy(self, a, x, y):
         _check(lib().qcd_axpy(self.h, a, _ptr(x), _ptr(y), x.numel(), _prec(x)))
@@ -229,20 +234,21 @@ class Context:
     def axpby(self, a, x, b, y):
         _check(lib().qcd_axpby(self.h, a, _ptr(x), b, _ptr(y), x.numel(), _prec(x)))
 
-    def norm2(self, x) -> float:
+    def norm2(self, x, fetch: bool = True):
         r = _d()
-        _check(lib().qcd_norm2(self.h, _ptr(x), x.numel(), _prec(x), C.byref(r)))
-        return r.value
+        _check(lib().qcd_norm2(self.h, _ptr(x), x.numel(), _prec(x), C.byref(r) if fetch else None))
+        return r.value if fetch else None
 
-    def redot(self, x, y) -> float:
+    def redot(self, x, y, fetch: bool = True):
         r = _d()
-        _check(lib().qcd_redot(self.h, _ptr(x), _ptr(y), x.numel(), _prec(x), C.byref(r)))
-        return r.value
+        _check(lib().qcd_redot(self.h, _ptr(x), _ptr(y), x.numel(), _prec(x), C.byref(r) if fetch else None))
+        return r.value if fetch else None
 
-    def cg_update(self, a, p, q, x, r) -> float:
+    def cg_update(self, a, p, q, x, r, fetch: bool = True):
         res = _d()
-        _check(lib().qcd_cg_update(self.h, a, _ptr(p), _ptr(q), _ptr(x), _ptr(r), x.numel(), _prec(x), C.byref(res)))
-        return res.value
+        _check(lib().qcd_cg_update(self.h, a, _ptr(p), _ptr(q), _ptr(x), _ptr(r), x.numel(), _prec(x),
+                                   C.byref(res) if fetch else None))
+        return res.value if fetch else None
 
     # ---- solvers -----------------------------------------------------------------------
     def set_operator(self, g_hi, g_lo=None, c_hi=None, c_lo=None, kappa=0.0, csw=0.0, parity=2, delta=0.1):
