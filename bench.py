@@ -225,13 +225,17 @@ def build_workload(c, dims, want_hi):
 
 
 def traffic_from_profile():
-    """dram bytes per launch of the dominant kernel from the committed ncu capture, if any."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    committed ncu --set full capture (profiles/traffic.csv); None if there is no capture."""
+    import csv
     try:
-        with open(p) as f:
-            return json.load(f).get("hop_clover_fp32_12_bytes_per_launch")
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["kernel"] == "hop_clover_fp32_12":
+                    return float(row["bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 def kernel_table(c, w, peak):
