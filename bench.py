@@ -299,6 +299,23 @@ def solver_table(c, w):
     return out
 
 
+def max_over_ranks(ms, device="cuda"):
+    """Multi-GPU timing rule: every rank contributes its device time, the job's time is the MAX
+    (replicas only: no data-path collective, this all-reduce is outside the timed region)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([float(ms)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(world, flop_per_step_per_rank, ms_step):
+    """Whole-job throughput of `world` independent replicas (weak scaling)."""
+    return world * flop_per_step_per_rank / (ms_step * 1e-3) * 1e-9
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -352,11 +369,9 @@ def run_ours(args):
     clocks = sampler.stop()
     if world > 1:
         dist.barrier()
-        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total)
     ms_step = ms_total / args.steps
-    value = world * step_flops(Vh) / (ms_step * 1e-3) * 1e-9
+    value = job_value(world, step_flops(Vh), ms_step)
 
     # ---- roofline of the dominant kernel (hop_kernel<float,12,*,CLOVER_*>): two launches per
     # step, algorithmic bytes 864 (clover-inverse epilogue) and 960 (clover + xpay) per site
@@ -385,11 +400,8 @@ def run_ours(args):
     e1.record()
     torch.cuda.synchronize()
     e2e_ms = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    e2e = {"value": round(world * step_flops(Vh) / (e2e_ms * 1e-3) * 1e-9, 1), "unit": UNIT,
+    e2e_ms = max_over_ranks(e2e_ms)
+    e2e = {"value": round(job_value(world, step_flops(Vh), e2e_ms), 1), "unit": UNIT,
            "h2d_bytes_per_step": blk_bytes, "d2h_bytes_per_step": blk_bytes, "ms_per_step": round(e2e_ms, 4),
            "steps": e2e_steps, "call": "qcd_dslash_host"}
 
