@@ -36,6 +36,7 @@ SMALL_DIMS = (16, 16, 16, 32)          # configs[1] lattice: the oracle's bounde
 EPS, KAPPA, CSW = 0.5, 0.1355, 1.0
 HOP_FLOP, CLOVER_FLOP = 1320.0, 504.0  # nominal flop / site (north_star)
 METRIC, UNIT = "wilson_clover_dslash_gflops", "GFLOP/s"
+TABLE_SCALE = 1.0
 
 
 def parse_args():
@@ -46,6 +47,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--quick", action="store_true", help="skip the per-kernel / solver sections")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-solvers", action="store_true", help="kernel table only (for ncu passes)")
+    ap.add_argument("--config4", action="store_true", help="also run the 48^3x96 Chebyshev workload (configs[4])")
+    ap.add_argument("--table-scale", type=float, default=1.0, help="scale the iteration counts of the kernel table")
     return ap.parse_args()
 
 
@@ -188,7 +192,8 @@ def gpu_time_ms(fn, iters, warm=3):
     """Average device time of fn() in ms: CUDA events on the launching stream (the ctx is
     bound to torch's current stream), after warm-up, synchronised on both sides."""
     import torch
-    for _ in range(warm):
+    iters = max(1, int(iters * TABLE_SCALE))
+    for _ in range(warm if TABLE_SCALE >= 1.0 else 1):
         fn()
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -296,6 +301,81 @@ def solver_table(c, w):
         out[name] = {"seconds": round(st.seconds, 5), "iters": st.iters, "reliable_updates": st.reliable_updates,
                      "r_true": st.r_true, "rc": rc, "GFLOP/s": round(st.flops / st.seconds * 1e-9, 1),
                      "ms_per_iter": round(st.seconds / max(st.iters, 1) * 1e3, 4)}
+    return out
+
+
+def config_table(c, peak, config4):
+    """The other BASELINE.json configs at their full sizes (parity for each is in tests/)."""
+    import torch
+    from paper_2001_05706_b200 import inputs
+    out = {}
+    # configs[1]: 16^3x32 fp32 even-odd Wilson, kappa 0.137, 18- and 12-real; single apply + 100-loop.
+    dims, kappa = (16, 16, 16, 32), 0.137
+    Vh = 16 * 16 * 16 * 32 // 2
+    h = Vh * 24
+    dU = torch.from_numpy(inputs.gauge_field(dims, EPS, 0)).cuda()
+    pin = c.spinor_pack(torch.from_numpy(inputs.spinor_field(dims, 0, 0)).float().cuda(), dims)
+    src, dst, tmp = pin[:h].clone(), torch.empty_like(pin[:h]), torch.empty_like(pin[:h])
+    for rec in (18, 12):
+        g = c.gauge_load(dU, dims, 4, rec, -1)
+        fn = lambda: c.dslash_ex(dst, src, g, None, kappa, 0.0, 0, 0, tmp)
+        loop_ms = gpu_time_ms(fn, 100)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); fn(); e1.record(); e1.synchronize()
+        flop = 2 * HOP_FLOP * Vh
+        byts = (2 * (48 + 8 * rec) + 24) * 4 * Vh
+        out["config1_wilson_eo_16x32_fp32_%d" % rec] = {
+            "single_apply_us": round(e0.elapsed_time(e1) * 1e3, 2), "loop100_us_per_apply": round(loop_ms * 1e3, 2),
+            "GFLOP/s": round(flop / (loop_ms * 1e-3) * 1e-9, 1), "GB/s": round(byts / (loop_ms * 1e-3) * 1e-9, 1),
+            "frac": round(byts / (loop_ms * 1e-3) * 1e-9 / peak, 4),
+            "note": "L2-resident (38-50 MB working set): the HBM fraction is not a roofline statement here"}
+    del dU
+    # configs[2]: 24^3x64 fp64 Wilson-clover CG, kappa 0.135, csw 1, tol 1e-10, maxiter 5000.
+    dims, kappa = (24, 24, 24, 64), 0.135
+    Vh = 24 * 24 * 24 * 64 // 2
+    h = Vh * 24
+    dU = torch.from_numpy(inputs.tiled_gauge_field(dims, EPS, 0, 16)).cuda()
+    g = c.gauge_load(dU, dims, 8, 18, -1)
+    del dU
+    cl = c.clover_build(g, kappa, CSW, 8)
+    b = c.spinor_pack(torch.from_numpy(inputs.spinor_field(dims, 0, 1)).cuda(), dims)
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    for name, mode in (("config2_clover_cg_24x64_fp64_evenodd", 0), ("config2_clover_cg_24x64_fp64_full", 2)):
+        c.set_operator(g, None, cl, None, kappa, CSW, mode)
+        bb = b[:h].clone() if mode == 0 else b
+        x = torch.empty_like(bb)
+        c.cg_solve(x, bb, 1e-10, 5000)
+        rc, st = c.cg_solve(x, bb, 1e-10, 5000)
+        out[name] = {"seconds": round(st.seconds, 5), "iters": st.iters, "r_true": st.r_true, "rc": rc,
+                     "GFLOP/s": round(st.flops / st.seconds * 1e-9, 1), "ms_per_iter": round(st.seconds / max(st.iters, 1) * 1e3, 4)}
+    del g, cl, b
+    if config4:
+        # configs[4]: degree-100 Chebyshev of H_W (kappa 0.2) on 12 Gaussian vectors, 48^3x96 fp32.
+        dims, kappa, scale, nvec = (48, 48, 48, 96), 0.2, 2.6, 12
+        V = 48 * 48 * 48 * 96
+        dU = torch.from_numpy(inputs.tiled_gauge_field(dims, EPS, 0, 8).astype("float32")).cuda()
+        g = c.gauge_load(dU, dims, 4, 12, -1)
+        del dU
+        coeff = inputs.chebyshev_sign_coefficients(100)
+        c.ensure_workspace(2 * V * 24 * 4)
+        vs = [torch.randn(V * 24, device="cuda", dtype=torch.float32) for _ in range(nvec)]
+        y = torch.empty_like(vs[0])
+        c.cheb_apply(y, vs[0], g, kappa, coeff[:4], scale)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for v in vs:
+            c.cheb_apply(y, v, g, kappa, coeff, scale)
+        e1.record(); e1.synchronize()
+        sec = e0.elapsed_time(e1) * 1e-3
+        launches = nvec * 100 * 2
+        byts = 1056.0 * (V // 2) * launches
+        out["config4_chebyshev_48x96_fp32_12vec_deg100"] = {
+            "seconds": round(sec, 4), "us_per_launch": round(sec / launches * 1e6, 2),
+            "GFLOP/s": round(HOP_FLOP * (V // 2) * launches / sec * 1e-9, 1), "GB/s": round(byts / sec * 1e-9, 1),
+            "frac": round(byts / sec * 1e-9 / peak, 4), "B/site": 1056,
+            "note": "vector at a time; hop + gamma5 + 3-term recurrence + y accumulation fused in one launch per parity"}
     return out
 
 
@@ -427,7 +507,11 @@ def run_ours(args):
         line["cpu_baseline"] = cpu_baseline()
     if full:
         line["kernels"] = kernel_table(c, w, peak)
-        line["cg"] = solver_table(c, w)
+        if not args.no_solvers:
+            line["cg"] = solver_table(c, w)
+            del w
+            torch.cuda.empty_cache()
+            line["configs"] = config_table(c, peak, args.config4)
     print(json.dumps(line))
     if world > 1:
         dist.barrier()
@@ -436,6 +520,7 @@ def run_ours(args):
 
 if __name__ == "__main__":
     a = parse_args()
+    TABLE_SCALE = a.table_scale
     if a.impl == "reference":
         run_reference(a)
     else:
