@@ -186,12 +186,21 @@ int qcd_cg_solve_ex(qcd_ctx* ctx, void* x, const void* b, double tol, int maxite
  * the high precision. */
 int qcd_apply_operator(qcd_ctx* ctx, void* out, const void* in, int flags);
 
-/* ---- Chebyshev driver (reading O8/S16) -----------
+/* ---- Chebyshev driver (reading O8/S16) ----
  * y = sum_{k=0}^{degree} coeff[k] T_k(H_W/scale) v,  H_W = gamma5 (1 - kappa H), full
- * lattice, forward three-term recurrence.  v, y: full internal fields in the gauge's
- * precision; coeff: HOST array of degree+1 doubles.  Uses the ctx workspace. */
+ * lattice.  Evaluated by the Clenshaw recurrence b_k = c_k v + 2 X b_{k+1} - b_{k+2},
+ * y = c_0 v + X b_1 - b_2 (the same polynomial as the forward three-term recurrence of
+ * reading O8, one operator apply per degree; gamma5, the recurrence and the coefficient
+ * term are fused into the hop kernel's epilogue: 2 launches per degree).
+ * v, y: full internal fields in the gauge's precision; coeff: HOST array of degree+1
+ * doubles.  Uses the ctx workspace (2 full fields per vector).
+ * qcd_cheb_apply_multi: nvec right-hand sides stored as nvec consecutive full fields in
+ * v and y; each link is read from HBM once per thread block and reused for all vectors
+ * (PAPER.md:68,109 multi-blas batching; PAPER.md:155 many-vector overlap workload). */
 int qcd_cheb_apply(qcd_ctx* ctx, void* y, const void* v, const qcd_gauge* g, double kappa,
                    const double* coeff, int degree, double scale);
+int qcd_cheb_apply_multi(qcd_ctx* ctx, void* y, const void* v, int nvec, const qcd_gauge* g,
+                         double kappa, const double* coeff, int degree, double scale);
 
 /* ---- host-buffer convenience (end-to-end path: copies inside the call) -------------
  * out_host = H_{p,1-p} in_host for one-parity blocks held in HOST memory, internal

@@ -22,16 +22,60 @@ template <typename T> struct HopArgs {
     T* out;
     const T* in;
     const T* z;
-    T* y;
-    T* tm;
+    const T* tm;   /* Chebyshev: b_{k+2}, own parity (may alias out)            */
+    const T* v;    /* Chebyshev: the source vector, own parity                  */
     const T* gauge;
     const T* clover;
     size_t gblock; /* reals per (mu, parity) gauge block */
+    size_t vstride; /* Chebyshev multi-rhs: reals between consecutive vectors   */
+    int nvec;
     DevGeom geo;
     int parity;
     T tb;
-    T a, b, c0, c1, c2, ck;
-    int y_init;
+    T a, b, c1, c2, c3;
+};
+
+/* ---- where a direction's link comes from ------------------------------------------- */
+template <typename T, int RECON> struct GlobalLinks {
+    const T* gauge;
+    size_t gblock, Vh;
+    int parity;
+    template <int MU, int DIR> __device__ __forceinline__ void get(T (&u)[18], int cb, int nb_cb) const
+    {
+        if (DIR > 0)
+            load_link<T, RECON>(u, gauge + (size_t)(2 * MU + parity) * gblock, Vh, (size_t)cb);
+        else
+            load_link<T, RECON>(u, gauge + (size_t)(2 * MU + (1 - parity)) * gblock, Vh, (size_t)nb_cb);
+    }
+};
+
+/* Per-thread slots in shared memory: slot (d, chunk) of thread tid at [(d*NCH + chunk)*128 + tid]
+ * (128-bit words) -> conflict-free LDS.128 / STS.128; only the owning thread touches its slots,
+ * so no barrier is needed.  Used by the multi-right-hand-side kernel to load each link from
+ * HBM once per block instead of once per vector. */
+template <typename T, int RECON> struct SmemLinks {
+    typedef typename Vec<T>::type V;
+    static constexpr int NCH = (RECON * (int)sizeof(T) + 15) / 16;
+    V* slot; /* = smem + threadIdx.x */
+    template <int MU, int DIR> __device__ __forceinline__ void put(const T (&u)[18]) const
+    {
+        constexpr int d = 2 * MU + (DIR < 0 ? 1 : 0);
+        T r[NCH * Vec<T>::reals];
+#pragma unroll
+        for (int i = 0; i < NCH * Vec<T>::reals; i++) r[i] = (i < RECON) ? u[i] : (T)0;
+#pragma unroll
+        for (int c = 0; c < NCH; c++) slot[(d * NCH + c) * 128] = vec_make(&r[c * Vec<T>::reals]);
+    }
+    template <int MU, int DIR> __device__ __forceinline__ void get(T (&u)[18], int, int) const
+    {
+        constexpr int d = 2 * MU + (DIR < 0 ? 1 : 0);
+        T r[NCH * Vec<T>::reals];
+#pragma unroll
+        for (int c = 0; c < NCH; c++) vec_get(slot[(d * NCH + c) * 128], &r[c * Vec<T>::reals]);
+#pragma unroll
+        for (int i = 0; i < RECON; i++) u[i] = r[i];
+        if (RECON == 12) reconstruct_row2<T>(u);
+    }
 };
 
 /* spin projection: h = rows 0,1 of (1 + S g_mu) psi.  s[2*(3*spin+col)+reim]; h[2*(3*j+col)+reim] */
@@ -124,16 +168,12 @@ __device__ __forceinline__ void colour_mul(T (&w)[12], const T (&u)[18], const T
 }
 
 /* one direction: MU, DIR = +1 forward / -1 backward; SG = projector sign (forward: -1, i.e. 1 - g) */
-template <typename T, int RECON, int MU, int DIR, int SG>
-__device__ __forceinline__ void hop_dir(T (&acc)[24], const HopArgs<T>& A, int cb, int nb_cb, T sign)
+template <typename T, int MU, int DIR, int SG, typename Links>
+__device__ __forceinline__ void hop_dir(T (&acc)[24], const Links& L, const T* __restrict__ in, size_t Vh, int cb, int nb_cb, T sign)
 {
-    const size_t Vh = (size_t)A.geo.Vh;
     T s[24], u[18], h[12], w[12];
-    load_planes<T, 24>(s, A.in, Vh, (size_t)nb_cb);
-    if (DIR > 0)
-        load_link<T, RECON>(u, A.gauge + (size_t)(2 * MU + A.parity) * A.gblock, Vh, (size_t)cb);
-    else
-        load_link<T, RECON>(u, A.gauge + (size_t)(2 * MU + (1 - A.parity)) * A.gblock, Vh, (size_t)nb_cb);
+    load_planes<T, 24>(s, in, Vh, (size_t)nb_cb);
+    L.template get<MU, DIR>(u, cb, nb_cb);
     project<T, MU, SG>(h, s);
     colour_mul<T, (DIR < 0)>(w, u, h, sign);
     reconstruct_add<T, MU, SG>(acc, w);
@@ -171,45 +211,57 @@ __device__ __forceinline__ void clover_apply(T (&o)[24], const T* __restrict__ c
     }
 }
 
+/* neighbour checkerboard indices (periodic wrap; reading S3) and t-seam signs (S4) */
+template <typename T> struct Neighbours {
+    int xp, xm, yp, ym, zp, zm, tp, tm;
+    T sgn_tp, sgn_tm;
+    __device__ __forceinline__ Neighbours(const DevGeom& g, int cb, int parity, T tb)
+    {
+        const Coord c = cb_to_coord(g, cb, parity);
+        const int odd = c.x & 1;
+        xp = odd ? (c.x == g.X - 1 ? cb - (g.X2 - 1) : cb + 1) : cb;
+        xm = odd ? cb : (c.x == 0 ? cb + (g.X2 - 1) : cb - 1);
+        const int sy = g.X2, sz = g.X2 * g.Y, st = g.X2 * g.Y * g.Z;
+        yp = (c.y == g.Y - 1) ? cb - (g.Y - 1) * sy : cb + sy;
+        ym = (c.y == 0) ? cb + (g.Y - 1) * sy : cb - sy;
+        zp = (c.z == g.Z - 1) ? cb - (g.Z - 1) * sz : cb + sz;
+        zm = (c.z == 0) ? cb + (g.Z - 1) * sz : cb - sz;
+        tp = (c.t == g.T - 1) ? cb - (g.T - 1) * st : cb + st;
+        tm = (c.t == 0) ? cb + (g.T - 1) * st : cb - st;
+        sgn_tp = (c.t == g.T - 1) ? tb : (T)1;
+        sgn_tm = (c.t == 0) ? tb : (T)1;
+    }
+};
+
+/* acc = (H in)(cb) (or H^dag): the eight directions */
+template <typename T, int DAG, typename Links>
+__device__ __forceinline__ void hop_site(T (&acc)[24], const Links& L, const T* __restrict__ in, size_t Vh, int cb, const Neighbours<T>& n)
+{
+    /* forward hop carries (1 - g_mu), backward (1 + g_mu); the adjoint swaps them (O4) */
+    constexpr int SF = DAG ? +1 : -1;
+    constexpr int SB = DAG ? -1 : +1;
+#pragma unroll
+    for (int i = 0; i < 24; i++) acc[i] = 0;
+    hop_dir<T, 0, +1, SF>(acc, L, in, Vh, cb, n.xp, (T)1);
+    hop_dir<T, 0, -1, SB>(acc, L, in, Vh, cb, n.xm, (T)1);
+    hop_dir<T, 1, +1, SF>(acc, L, in, Vh, cb, n.yp, (T)1);
+    hop_dir<T, 1, -1, SB>(acc, L, in, Vh, cb, n.ym, (T)1);
+    hop_dir<T, 2, +1, SF>(acc, L, in, Vh, cb, n.zp, (T)1);
+    hop_dir<T, 2, -1, SB>(acc, L, in, Vh, cb, n.zm, (T)1);
+    hop_dir<T, 3, +1, SF>(acc, L, in, Vh, cb, n.tp, n.sgn_tp);
+    hop_dir<T, 3, -1, SB>(acc, L, in, Vh, cb, n.tm, n.sgn_tm);
+}
+
 template <typename T, int RECON, int DAG, int MODE>
 __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_kernel(const HopArgs<T> A)
 {
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= A.geo.Vh) return;
-    const DevGeom& g = A.geo;
-    const Coord c = cb_to_coord(g, cb, A.parity);
-    const size_t Vh = (size_t)g.Vh;
-
-    /* neighbour checkerboard indices (periodic wrap; reading S3) */
-    const int odd = c.x & 1;
-    const int xp = odd ? (c.x == g.X - 1 ? cb - (g.X2 - 1) : cb + 1) : cb;
-    const int xm = odd ? cb : (c.x == 0 ? cb + (g.X2 - 1) : cb - 1);
-    const int sy = g.X2, sz = g.X2 * g.Y, st = g.X2 * g.Y * g.Z;
-    const int yp = (c.y == g.Y - 1) ? cb - (g.Y - 1) * sy : cb + sy;
-    const int ym = (c.y == 0) ? cb + (g.Y - 1) * sy : cb - sy;
-    const int zp = (c.z == g.Z - 1) ? cb - (g.Z - 1) * sz : cb + sz;
-    const int zm = (c.z == 0) ? cb + (g.Z - 1) * sz : cb - sz;
-    const int tp = (c.t == g.T - 1) ? cb - (g.T - 1) * st : cb + st;
-    const int tmn = (c.t == 0) ? cb + (g.T - 1) * st : cb - st;
-    const T sgn_tp = (c.t == g.T - 1) ? A.tb : (T)1;
-    const T sgn_tm = (c.t == 0) ? A.tb : (T)1;
-
-    /* forward hop carries (1 - g_mu), backward (1 + g_mu); the adjoint swaps them (O4) */
-    constexpr int SF = DAG ? +1 : -1;
-    constexpr int SB = DAG ? -1 : +1;
-
+    const size_t Vh = (size_t)A.geo.Vh;
+    const Neighbours<T> nb(A.geo, cb, A.parity, A.tb);
+    const GlobalLinks<T, RECON> L = {A.gauge, A.gblock, Vh, A.parity};
     T acc[24];
-#pragma unroll
-    for (int i = 0; i < 24; i++) acc[i] = 0;
-
-    hop_dir<T, RECON, 0, +1, SF>(acc, A, cb, xp, (T)1);
-    hop_dir<T, RECON, 0, -1, SB>(acc, A, cb, xm, (T)1);
-    hop_dir<T, RECON, 1, +1, SF>(acc, A, cb, yp, (T)1);
-    hop_dir<T, RECON, 1, -1, SB>(acc, A, cb, ym, (T)1);
-    hop_dir<T, RECON, 2, +1, SF>(acc, A, cb, zp, (T)1);
-    hop_dir<T, RECON, 2, -1, SB>(acc, A, cb, zm, (T)1);
-    hop_dir<T, RECON, 3, +1, SF>(acc, A, cb, tp, sgn_tp);
-    hop_dir<T, RECON, 3, -1, SB>(acc, A, cb, tmn, sgn_tm);
+    hop_site<T, DAG>(acc, L, A.in, Vh, cb, nb);
 
     if (MODE == HOP_PLAIN) {
         store_planes<T, 24>(A.out, Vh, (size_t)cb, acc);
@@ -230,31 +282,74 @@ __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_kernel(cons
         T o[24];
         clover_apply<T>(o, A.clover, Vh, (size_t)cb, acc);
         store_planes<T, 24>(A.out, Vh, (size_t)cb, o);
-    } else { /* HOP_CHEB: tn = c1 g5 (z + b H in) + c2 tm ; y (+)= ck tn ; tm <- tn  (reading O8) */
-        T zz[24], yy[24];
-        load_planes_rw<T, 24>(zz, A.z, Vh, (size_t)cb);
+    }
+}
+
+/* ---- Chebyshev (Clenshaw) step for nvec right-hand sides -----
+ *   out_j = c1 g5 (z_j + b H in_j) + c2 tm_j + c3 v_j          j = 0 .. nvec-1
+ * with z_j the own-parity block of the field whose other-parity block is in_j.  The block's
+ * 8 x 128 links are read from HBM once, parked in per-thread shared-memory slots and reused
+ * for every vector, so the link traffic per site-vector is 8*RECON reals / nvec.  out may alias
+ * tm (same index, same thread). */
+template <typename T, int RECON>
+__global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_cheb_mrhs_kernel(const HopArgs<T> A)
+{
+    typedef typename Vec<T>::type V;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= A.geo.Vh) return;
+    const size_t Vh = (size_t)A.geo.Vh;
+    const Neighbours<T> nb(A.geo, cb, A.parity, A.tb);
+    const GlobalLinks<T, RECON> G = {A.gauge, A.gblock, Vh, A.parity};
+    const SmemLinks<T, RECON> S = {reinterpret_cast<V*>(smem_raw) + threadIdx.x};
+    {
+        T u[18];
+        G.template get<0, +1>(u, cb, nb.xp); S.template put<0, +1>(u);
+        G.template get<0, -1>(u, cb, nb.xm); S.template put<0, -1>(u);
+        G.template get<1, +1>(u, cb, nb.yp); S.template put<1, +1>(u);
+        G.template get<1, -1>(u, cb, nb.ym); S.template put<1, -1>(u);
+        G.template get<2, +1>(u, cb, nb.zp); S.template put<2, +1>(u);
+        G.template get<2, -1>(u, cb, nb.zm); S.template put<2, -1>(u);
+        G.template get<3, +1>(u, cb, nb.tp); S.template put<3, +1>(u);
+        G.template get<3, -1>(u, cb, nb.tm); S.template put<3, -1>(u);
+    }
+    for (int j = 0; j < A.nvec; j++) {
+        const size_t off = (size_t)j * A.vstride;
+        T acc[24], zz[24];
+        hop_site<T, 0>(acc, S, A.in + off, Vh, cb, nb);
+        load_planes<T, 24>(zz, A.z + off, Vh, (size_t)cb);
 #pragma unroll
         for (int i = 0; i < 24; i++) {
             const T g5 = (i < 12) ? (T)1 : (T)-1; /* gamma5 = diag(1,1,-1,-1) */
             acc[i] = A.c1 * g5 * (zz[i] + A.b * acc[i]);
         }
+        if (A.c3 != (T)0) {
+            load_planes<T, 24>(zz, A.v + off, Vh, (size_t)cb);
+#pragma unroll
+            for (int i = 0; i < 24; i++) acc[i] += A.c3 * zz[i];
+        }
         if (A.c2 != (T)0) {
-            T tt[24];
-            load_planes_rw<T, 24>(tt, A.tm, Vh, (size_t)cb);
+            load_planes_rw<T, 24>(zz, A.tm + off, Vh, (size_t)cb);
 #pragma unroll
-            for (int i = 0; i < 24; i++) acc[i] += A.c2 * tt[i];
+            for (int i = 0; i < 24; i++) acc[i] += A.c2 * zz[i];
         }
-        if (A.y_init) {
-#pragma unroll
-            for (int i = 0; i < 24; i++) yy[i] = A.c0 * zz[i] + A.ck * acc[i];
-        } else {
-            load_planes_rw<T, 24>(yy, A.y, Vh, (size_t)cb);
-#pragma unroll
-            for (int i = 0; i < 24; i++) yy[i] += A.ck * acc[i];
-        }
-        store_planes<T, 24>(A.y, Vh, (size_t)cb, yy);
-        store_planes<T, 24>(A.tm, Vh, (size_t)cb, acc);
+        store_planes<T, 24>(A.out + off, Vh, (size_t)cb, acc);
     }
+}
+
+template <typename T, int RECON> static cudaError_t hop_cheb_launch(const HopArgs<T>& A, cudaStream_t st)
+{
+    const int threads = 128;
+    const int blocks = (A.geo.Vh + threads - 1) / threads;
+    const size_t smem = (size_t)8 * SmemLinks<T, RECON>::NCH * 128 * 16;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(hop_cheb_mrhs_kernel<T, RECON>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    hop_cheb_mrhs_kernel<T, RECON><<<blocks, threads, smem, st>>>(A);
+    return cudaGetLastError();
 }
 
 template <typename T, int RECON, int DAG> static cudaError_t hop_dispatch_mode(const HopArgs<T>& A, int mode, cudaStream_t st)
@@ -266,7 +361,6 @@ template <typename T, int RECON, int DAG> static cudaError_t hop_dispatch_mode(c
     case HOP_XPAY: hop_kernel<T, RECON, DAG, HOP_XPAY><<<blocks, threads, 0, st>>>(A); break;
     case HOP_CLOVER_Z: hop_kernel<T, RECON, DAG, HOP_CLOVER_Z><<<blocks, threads, 0, st>>>(A); break;
     case HOP_CLOVER_OUT: hop_kernel<T, RECON, DAG, HOP_CLOVER_OUT><<<blocks, threads, 0, st>>>(A); break;
-    case HOP_CHEB: hop_kernel<T, RECON, DAG, HOP_CHEB><<<blocks, threads, 0, st>>>(A); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
@@ -274,6 +368,7 @@ template <typename T, int RECON, int DAG> static cudaError_t hop_dispatch_mode(c
 
 template <typename T> static cudaError_t hop_dispatch(const HopArgs<T>& A, int recon, int dagger, int mode, cudaStream_t st)
 {
+    if (mode == HOP_CHEB) return recon == 12 ? hop_cheb_launch<T, 12>(A, st) : hop_cheb_launch<T, 18>(A, st);
     if (recon == 12)
         return dagger ? hop_dispatch_mode<T, 12, 1>(A, mode, st) : hop_dispatch_mode<T, 12, 0>(A, mode, st);
     return dagger ? hop_dispatch_mode<T, 18, 1>(A, mode, st) : hop_dispatch_mode<T, 18, 0>(A, mode, st);
@@ -285,16 +380,17 @@ template <typename T> static HopArgs<T> make_hop_args(const qcd_gauge* g, const 
     A.out = (T*)L.out;
     A.in = (const T*)L.in;
     A.z = (const T*)L.z;
-    A.y = (T*)L.y;
-    A.tm = (T*)L.tm;
+    A.tm = (const T*)L.tm;
+    A.v = (const T*)L.v;
+    A.vstride = L.vstride;
+    A.nvec = L.nvec;
     A.gauge = (const T*)g->data;
     A.clover = (const T*)L.clover;
     A.gblock = g->block_bytes / sizeof(T);
     A.geo = dev_geom(g->geo);
     A.parity = L.out_parity;
     A.tb = (T)g->tb;
-    A.a = (T)L.a; A.b = (T)L.b; A.c0 = (T)L.c0; A.c1 = (T)L.c1; A.c2 = (T)L.c2; A.ck = (T)L.ck;
-    A.y_init = L.y_init;
+    A.a = (T)L.a; A.b = (T)L.b; A.c1 = (T)L.c1; A.c2 = (T)L.c2; A.c3 = (T)L.c3;
     return A;
 }
 

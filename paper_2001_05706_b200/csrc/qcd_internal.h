@@ -89,19 +89,19 @@ enum HopMode {
     HOP_XPAY = 1,        /* out = a z + b H in                                    */
     HOP_CLOVER_Z = 2,    /* out = a (A z) + b H in                                */
     HOP_CLOVER_OUT = 3,  /* out = Ainv (H in)                                     */
-    HOP_CHEB = 4         /* tn = c1 g5 (z + b H in) + c2 tm; y (+)= ck tn; tm = tn */
+    HOP_CHEB = 4         /* out_j = c1 g5 (z_j + b H in_j) + c2 tm_j + c3 v_j, j < nvec */
 };
 
 struct HopLaunch {
-    void* out;            /* one-parity block (cheb: unused)                      */
+    void* out;            /* one-parity block                                     */
     const void* in;       /* other-parity block                                   */
     const void* z;        /* own-parity block (modes 1,2,4)                       */
-    void* y;              /* cheb accumulator, own parity                         */
-    void* tm;             /* cheb T_{k-1} in / T_{k+1} out, own parity            */
+    const void* tm;       /* cheb: b_{k+2}, own parity (may alias out)            */
+    const void* v;        /* cheb: source vector, own parity                      */
     const void* clover;   /* A or A^-1 block of the output parity (modes 2,3)     */
-    double a, b, c1, c2, ck;
-    int y_init;           /* cheb: y = c0 z + ck tn instead of y += ck tn         */
-    double c0;
+    double a, b, c1, c2, c3;
+    size_t vstride;       /* cheb: reals between consecutive right-hand sides     */
+    int nvec;             /* cheb: number of right-hand sides                     */
     int out_parity, dagger, mode;
 };
 

@@ -278,45 +278,60 @@ int qcd_cg_solve(void* x, const void* b, double tol, int maxiter)
     return qcd_cg_solve_ex(g_last_ctx, x, b, tol, maxiter, nullptr);
 }
 
-int qcd_cheb_apply(qcd_ctx* ctx, void* y, const void* v, const qcd_gauge* g, double kappa, const double* coeff, int degree, double scale)
+int qcd_cheb_apply_multi(qcd_ctx* ctx, void* y, const void* v, int nvec, const qcd_gauge* g, double kappa, const double* coeff,
+                         int degree, double scale)
 {
     QCD_REQUIRE(ctx && g && y && v && coeff, "cheb_apply: NULL argument");
-    QCD_REQUIRE(degree >= 0 && scale > 0.0, "cheb_apply: degree must be >= 0 and scale > 0");
-    QCD_REQUIRE(y != v, "cheb_apply: y and v alias");
+    QCD_REQUIRE(degree >= 0 && scale > 0.0 && nvec >= 1, "cheb_apply: degree must be >= 0, scale > 0, nvec >= 1");
+    QCD_REQUIRE((((uintptr_t)y | (uintptr_t)v) & 15u) == 0, "cheb_apply: y/v must be 16-byte aligned");
     const int P = g->precision;
     const size_t blk = (size_t)g->geo.Vh * 24 * P, full = 2 * blk, nreal = (size_t)g->geo.V * 24;
-    QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= 2 * full, "cheb_apply: workspace too small (need %zu bytes)", 2 * full);
-    char* ta = (char*)ctx->ws;
-    char* tb = ta + full;
-    if (degree == 0) {
-        RC(blas_copy(ctx, y, v, full));
-        return blas_axpby(ctx, host_scalar(0.0), v, host_scalar(coeff[0]), y, nreal, P);
+    const size_t batch = (size_t)nvec * full;
+    {
+        const uintptr_t a0 = (uintptr_t)y, a1 = (uintptr_t)v;
+        QCD_REQUIRE(a0 + batch <= a1 || a1 + batch <= a0, "cheb_apply: y and v alias");
     }
-    RC(blas_copy(ctx, tb, v, full)); /* T_0 */
-    char* tk = tb;  /* T_k     */
-    char* tkm = ta; /* T_{k-1}, overwritten by T_{k+1} */
-    for (int k = 0; k < degree; k++) {
+    if (degree == 0) {
+        RC(blas_copy(ctx, y, v, batch));
+        return blas_axpby(ctx, host_scalar(0.0), v, host_scalar(coeff[0]), y, nreal * nvec, P);
+    }
+    QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= 2 * batch, "cheb_apply: workspace too small (need %zu bytes)", 2 * batch);
+    /* Clenshaw: b_{d+1} = b_{d+2} = 0; b_k = c_k v + 2 X b_{k+1} - b_{k+2}; y = c_0 v + X b_1 - b_2,
+     * X = g5 (1 - kappa H) / scale.  b_d = c_d v needs no operator apply. */
+    char* bk1 = (char*)ctx->ws;  /* b_{k+1} */
+    char* bk2 = bk1 + batch;     /* b_{k+2}, overwritten by b_k */
+    RC(blas_copy(ctx, bk1, v, batch));
+    RC(blas_axpby(ctx, host_scalar(0.0), v, host_scalar(coeff[degree]), bk1, nreal * nvec, P));
+    for (int k = degree - 1; k >= 0; k--) {
+        const bool first = (k == degree - 1), last = (k == 0);
+        char* out = last ? (char*)y : bk2;
         for (int p = 0; p < 2; p++) {
             HopLaunch L;
             memset(&L, 0, sizeof(L));
             L.mode = HOP_CHEB;
-            L.in = tk + (1 - p) * blk;
-            L.z = tk + p * blk;
-            L.tm = tkm + p * blk;
-            L.y = (char*)y + p * blk;
+            L.in = bk1 + (1 - p) * blk;
+            L.z = bk1 + p * blk;
+            L.tm = bk2 + p * blk;
+            L.v = (const char*)v + p * blk;
+            L.out = out + p * blk;
             L.b = -kappa;
-            L.c1 = (k == 0 ? 1.0 : 2.0) / scale;
-            L.c2 = (k == 0 ? 0.0 : -1.0);
-            L.ck = coeff[k + 1];
-            L.y_init = (k == 0);
-            L.c0 = coeff[0];
+            L.c1 = (last ? 1.0 : 2.0) / scale;
+            L.c2 = first ? 0.0 : -1.0;
+            L.c3 = coeff[k];
+            L.vstride = nreal;
+            L.nvec = nvec;
             L.out_parity = p;
             L.dagger = 0;
             RC(hop_launch(ctx, g, L));
         }
-        char* s = tk; tk = tkm; tkm = s;
+        if (!last) { char* s = bk1; bk1 = bk2; bk2 = s; }
     }
     return QCD_OK;
+}
+
+int qcd_cheb_apply(qcd_ctx* ctx, void* y, const void* v, const qcd_gauge* g, double kappa, const double* coeff, int degree, double scale)
+{
+    return qcd_cheb_apply_multi(ctx, y, v, 1, g, kappa, coeff, degree, scale);
 }
 
 } /* extern "C" */

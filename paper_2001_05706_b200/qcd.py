@@ -72,6 +72,7 @@ SIGNATURES = {
     "qcd_cg_solve_ex": (_i, [_vp, _vp, _vp, _d, _i, C.POINTER(Stats)]),
     "qcd_apply_operator": (_i, [_vp, _vp, _vp, _i]),
     "qcd_cheb_apply": (_i, [_vp, _vp, _vp, _vp, _d, C.POINTER(_d), _i, _d]),
+    "qcd_cheb_apply_multi": (_i, [_vp, _vp, _vp, _i, _vp, _d, C.POINTER(_d), _i, _d]),
     "qcd_hop_host": (_i, [_vp, _vp, _vp, _vp, _i, _i]),
     "qcd_dslash_host": (_i, [_vp, _vp, _vp, _vp, _vp, _d, _d, _i, _i]),
     "qcd_launch_count": (C.c_longlong, [_vp]),
@@ -269,6 +270,12 @@ class Context:
         n = len(coeff)
         arr = (_d * n)(*[float(c) for c in coeff])
         _check(lib().qcd_cheb_apply(self.h, _ptr(y), _ptr(v), gauge.h, kappa, arr, n - 1, scale))
+
+    def cheb_apply_multi(self, y, v, nvec: int, gauge: "Gauge", kappa: float, coeff, scale: float):
+        """y, v: nvec consecutive full internal fields."""
+        n = len(coeff)
+        arr = (_d * n)(*[float(c) for c in coeff])
+        _check(lib().qcd_cheb_apply_multi(self.h, _ptr(y), _ptr(v), nvec, gauge.h, kappa, arr, n - 1, scale))
 
     def launch_count(self) -> int:
         return int(lib().qcd_launch_count(self.h))
