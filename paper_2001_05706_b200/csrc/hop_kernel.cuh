@@ -29,6 +29,7 @@ template <typename T> struct HopArgs {
     size_t gblock; /* reals per (mu, parity) gauge block */
     size_t vstride; /* Chebyshev multi-rhs: reals between consecutive vectors   */
     int nvec;
+    int tblock;     /* multi-rhs: t extent of the traversal tile (divides T)      */
     DevGeom geo;
     int parity;
     T tb;
@@ -291,16 +292,57 @@ __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_kernel(cons
  * 8 x 128 links are read from HBM once, parked in per-thread shared-memory slots and reused
  * for every vector, so the link traffic per site-vector is 8*RECON reals / nvec.  out may alias
  * tm (same index, same thread). */
-template <typename T, int RECON>
+template <typename T, typename Links>
+__device__ __forceinline__ void cheb_vector(const HopArgs<T>& A, const Links& L, size_t off, size_t Vh, int cb, const Neighbours<T>& nb)
+{
+    T acc[24], zz[24];
+    hop_site<T, 0>(acc, L, A.in + off, Vh, cb, nb);
+    load_planes_cs<T, 24>(zz, A.z + off, Vh, (size_t)cb);
+#pragma unroll
+    for (int i = 0; i < 24; i++) {
+        const T g5 = (i < 12) ? (T)1 : (T)-1; /* gamma5 = diag(1,1,-1,-1) */
+        acc[i] = A.c1 * g5 * (zz[i] + A.b * acc[i]);
+    }
+    if (A.c3 != (T)0) {
+        load_planes_cs<T, 24>(zz, A.v + off, Vh, (size_t)cb);
+#pragma unroll
+        for (int i = 0; i < 24; i++) acc[i] += A.c3 * zz[i];
+    }
+    if (A.c2 != (T)0) {
+        load_planes_cs<T, 24>(zz, A.tm + off, Vh, (size_t)cb);
+#pragma unroll
+        for (int i = 0; i < 24; i++) acc[i] += A.c2 * zz[i];
+    }
+    store_planes_cs<T, 24>(A.out + off, Vh, (size_t)cb, acc);
+}
+
+/* STAGE = 1: nvec > 1, links parked in shared memory; STAGE = 0: one vector, links straight from HBM */
+template <typename T, int RECON, int STAGE>
 __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_cheb_mrhs_kernel(const HopArgs<T> A)
 {
     typedef typename Vec<T>::type V;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= A.geo.Vh) return;
+    if (STAGE && A.tblock > 1) {
+        /* Traversal order (x,y) fastest, then t inside a tile of tblock slices, then z, then the
+         * tiles: with nvec vectors in flight the L2 footprint between the two uses of a +-t
+         * neighbour is nvec planes instead of nvec time-slices, and between +-z uses nvec*tblock
+         * planes; only the tile faces in t are fetched twice. */
+        const unsigned P = (unsigned)(A.geo.X2 * A.geo.Y), TB = (unsigned)A.tblock, Z = (unsigned)A.geo.Z;
+        unsigned r = (unsigned)cb;
+        const unsigned xy = r % P; r /= P;
+        const unsigned tin = r % TB; r /= TB;
+        const unsigned z = r % Z; const unsigned tout = r / Z;
+        cb = (int)(xy + P * (z + Z * (tout * TB + tin)));
+    }
     const size_t Vh = (size_t)A.geo.Vh;
     const Neighbours<T> nb(A.geo, cb, A.parity, A.tb);
     const GlobalLinks<T, RECON> G = {A.gauge, A.gblock, Vh, A.parity};
+    if (!STAGE) {
+        cheb_vector<T>(A, G, 0, Vh, cb, nb);
+        return;
+    }
     const SmemLinks<T, RECON> S = {reinterpret_cast<V*>(smem_raw) + threadIdx.x};
     {
         T u[18];
@@ -313,42 +355,25 @@ __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_cheb_mrhs_k
         G.template get<3, +1>(u, cb, nb.tp); S.template put<3, +1>(u);
         G.template get<3, -1>(u, cb, nb.tm); S.template put<3, -1>(u);
     }
-    for (int j = 0; j < A.nvec; j++) {
-        const size_t off = (size_t)j * A.vstride;
-        T acc[24], zz[24];
-        hop_site<T, 0>(acc, S, A.in + off, Vh, cb, nb);
-        load_planes<T, 24>(zz, A.z + off, Vh, (size_t)cb);
-#pragma unroll
-        for (int i = 0; i < 24; i++) {
-            const T g5 = (i < 12) ? (T)1 : (T)-1; /* gamma5 = diag(1,1,-1,-1) */
-            acc[i] = A.c1 * g5 * (zz[i] + A.b * acc[i]);
-        }
-        if (A.c3 != (T)0) {
-            load_planes<T, 24>(zz, A.v + off, Vh, (size_t)cb);
-#pragma unroll
-            for (int i = 0; i < 24; i++) acc[i] += A.c3 * zz[i];
-        }
-        if (A.c2 != (T)0) {
-            load_planes_rw<T, 24>(zz, A.tm + off, Vh, (size_t)cb);
-#pragma unroll
-            for (int i = 0; i < 24; i++) acc[i] += A.c2 * zz[i];
-        }
-        store_planes<T, 24>(A.out + off, Vh, (size_t)cb, acc);
-    }
+    for (int j = 0; j < A.nvec; j++) cheb_vector<T>(A, S, (size_t)j * A.vstride, Vh, cb, nb);
 }
 
 template <typename T, int RECON> static cudaError_t hop_cheb_launch(const HopArgs<T>& A, cudaStream_t st)
 {
     const int threads = 128;
     const int blocks = (A.geo.Vh + threads - 1) / threads;
+    if (A.nvec == 1) {
+        hop_cheb_mrhs_kernel<T, RECON, 0><<<blocks, threads, 0, st>>>(A);
+        return cudaGetLastError();
+    }
     const size_t smem = (size_t)8 * SmemLinks<T, RECON>::NCH * 128 * 16;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(hop_cheb_mrhs_kernel<T, RECON>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(hop_cheb_mrhs_kernel<T, RECON, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    hop_cheb_mrhs_kernel<T, RECON><<<blocks, threads, smem, st>>>(A);
+    hop_cheb_mrhs_kernel<T, RECON, 1><<<blocks, threads, smem, st>>>(A);
     return cudaGetLastError();
 }
 
@@ -384,6 +409,9 @@ template <typename T> static HopArgs<T> make_hop_args(const qcd_gauge* g, const 
     A.v = (const T*)L.v;
     A.vstride = L.vstride;
     A.nvec = L.nvec;
+    A.tblock = 1;
+    for (int tbk = 16; tbk > 1; tbk >>= 1)
+        if (g->geo.T % tbk == 0 && g->geo.T > tbk) { A.tblock = tbk; break; }
     A.gauge = (const T*)g->data;
     A.clover = (const T*)L.clover;
     A.gblock = g->block_bytes / sizeof(T);

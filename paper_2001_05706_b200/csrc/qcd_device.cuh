@@ -60,6 +60,28 @@ __device__ __forceinline__ void load_planes_rw(T (&d)[NREAL], const T* base, siz
         vec_get(v, &d[c * Vec<T>::reals]);
     }
 }
+/* streaming variants (ld.global.cs / st.global.cs): data touched once per launch, marked
+ * evict-first so that it does not displace the neighbour spinors that L2 must keep for reuse */
+template <typename T, int NREAL>
+__device__ __forceinline__ void load_planes_cs(T (&d)[NREAL], const T* base, size_t stride, size_t idx)
+{
+    typedef typename Vec<T>::type V;
+    const V* p = reinterpret_cast<const V*>(base) + idx;
+#pragma unroll
+    for (int c = 0; c < NREAL / Vec<T>::reals; c++) {
+        V v = __ldcs(p + (size_t)c * stride);
+        vec_get(v, &d[c * Vec<T>::reals]);
+    }
+}
+template <typename T, int NREAL>
+__device__ __forceinline__ void store_planes_cs(T* base, size_t stride, size_t idx, const T (&d)[NREAL])
+{
+    typedef typename Vec<T>::type V;
+    V* p = reinterpret_cast<V*>(base) + idx;
+#pragma unroll
+    for (int c = 0; c < NREAL / Vec<T>::reals; c++) __stcs(p + (size_t)c * stride, vec_make(&d[c * Vec<T>::reals]));
+}
+
 template <typename T, int NREAL>
 __device__ __forceinline__ void store_planes(T* base, size_t stride, size_t idx, const T (&d)[NREAL])
 {

@@ -200,7 +200,7 @@ def test_chebyshev_multi_rhs_matches_oracle(precision, recon, dims):
     for i, v in enumerate(vs):
         want = orc.cheb(v, U, dims, kappa, coeff, scale)
         assert relerr(unpack(c, y[i * n:(i + 1) * n].contiguous(), dims), want) <= TOL[precision]
-    # one vector through the batched entry point == the single-vector entry point, bit for bit
+    # the single-vector entry point (links straight from HBM, no staging) agrees with the batch
     y1 = torch.empty_like(batch[:n])
     c.cheb_apply(y1, batch[:n].contiguous(), g, kappa, coeff, scale)
-    assert torch.equal(y1, y[:n])
+    assert relerr(y1.cpu().numpy(), y[:n].cpu().numpy()) <= (1e-6 if precision == 4 else 1e-14)
