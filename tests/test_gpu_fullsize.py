@@ -128,3 +128,98 @@ def test_operator_adjoint_identity_32x64(world):
     lhs, rhs = c.redot(chi, Mpsi), c.redot(Mdchi, src)
     scale = np.sqrt(c.norm2(chi) * c.norm2(Mpsi))
     assert abs(lhs - rhs) <= 2e-6 * scale
+
+
+# ---- the other configs at their full sizes ------------------------------------------------
+def _host_mem_gb():
+    try:
+        import psutil
+        return psutil.virtual_memory().available / 1e9
+    except Exception:
+        return 0.0
+
+
+def test_config2_clover_cg_24x64_fp64_full_size():
+    """BASELINE.json configs[2] as stated (24^3 x 64, fp64, kappa 0.135, csw 1, tol 1e-10,
+    maxiter 5000), even-odd form: iteration count within +-2 of the oracle, true residual
+    below tol, solution equal to the oracle's."""
+    if _host_mem_gb() < 24:
+        pytest.skip("needs ~20 GB of host memory for the oracle's dense clover field")
+    c = ctx()
+    dims, kappa, csw, tol = (24, 24, 24, 64), 0.135, 1.0, 1e-10
+    U = inputs.tiled_gauge_field(dims, 0.5, 0, 16)
+    A = orc.clover_matrix(orc.field_strength(U, dims), dims, kappa * csw)
+    Ainv = orc.invert_12(A)
+    par = orc.parity_mask_array(dims)[..., None, None, None]
+    b = inputs.spinor_field(dims, 0, 1) * (par == 0)
+    x_ref, st_ref = orc.cg(b, U, dims, kappa, tol, 5000, A, Ainv, -1, 0)
+    g = c.gauge_load(torch.from_numpy(U).cuda(), dims, 8, 18, -1)
+    cl = c.clover_build(g, kappa, csw, 8)
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    c.set_operator(g, None, cl, None, kappa, csw, 0)
+    pb = c.spinor_pack(torch.from_numpy(b).cuda(), dims)
+    h = pb.numel() // 2
+    full = torch.zeros_like(pb)
+    rc, st = c.cg_solve(full[:h], pb[:h], tol, 5000)
+    assert rc == 0 and st.converged == 1
+    assert abs(st.iters - st_ref["iters"]) <= 2
+    assert st.r_true < 1.5 * tol
+    assert relerr(c.spinor_unpack(full, dims).cpu().numpy(), x_ref) <= 1e-8
+
+
+def test_config3_mixed_cg_32x64_full_size(world):
+    """BASELINE.json configs[3] as stated (32^3 x 64, fp32 12-real inner / fp64 outer reliable
+    updates, kappa 0.1355, csw 1, tol 1e-10), even-odd form, against the oracle's mixed CG."""
+    if _host_mem_gb() < 60:
+        pytest.skip("needs ~50 GB of host memory for the oracle's dense fp64 + fp32 clover fields")
+    c = ctx()
+    tol = 1e-10
+    U = inputs.tiled_gauge_field(DIMS, 0.5, 0, 16)
+    A = orc.clover_matrix(orc.field_strength(U, DIMS), DIMS, KAPPA * CSW)
+    Ainv = orc.invert_12(A)
+    par = orc.parity_mask_array(DIMS)[..., None, None, None]
+    b = inputs.spinor_field(DIMS, 0, 1) * (par == 0)
+    y_ref, st_ref = orc.cg_mixed(b, U, DIMS, KAPPA, tol, 5000, A, Ainv, -1, 0, 0.1)
+    del A, Ainv
+    dU = torch.from_numpy(U).cuda()
+    g_hi = c.gauge_load(dU, DIMS, 8, 18, -1)
+    g_lo = c.gauge_load(dU, DIMS, 4, 12, -1)
+    del dU
+    c_hi = c.clover_build(g_hi, KAPPA, CSW, 8)
+    c_lo = c.clover_build(g_hi, KAPPA, CSW, 4)
+    c.ensure_workspace(c.workspace_bytes(DIMS, 8))
+    c.set_operator(g_hi, g_lo, c_hi, c_lo, KAPPA, CSW, 0, 0.1)
+    pb = c.spinor_pack(torch.from_numpy(b).cuda(), DIMS)
+    h = pb.numel() // 2
+    full = torch.zeros_like(pb)
+    rc, st = c.cg_solve(full[:h], pb[:h], tol, 5000)
+    assert rc == 0 and st.converged == 1
+    assert abs(st.iters - st_ref["iters"]) <= 2
+    assert abs(st.reliable_updates - st_ref["reliable_updates"]) <= 1
+    assert st.r_true < 1.5 * tol
+    assert relerr(c.spinor_unpack(full, DIMS).cpu().numpy(), y_ref) <= 1e-8
+
+
+def test_config4_chebyshev_48x96_reduced_degree_full_size():
+    """BASELINE.json configs[4] lattice (48^3 x 96, fp32, 12-real, kappa 0.2): the oracle is too
+    slow for degree 100 x 12 vectors at this size, so the full-size check is
+    degree 4 on 2 vectors through the multi-rhs entry point, whole field compared."""
+    if _host_mem_gb() < 40:
+        pytest.skip("needs ~30 GB of host memory")
+    c = ctx()
+    dims, kappa, scale = (48, 48, 48, 96), 0.2, 2.6
+    U = inputs.round_to_f32(inputs.tiled_gauge_field(dims, 0.5, 0, 8))
+    coeff = inputs.chebyshev_sign_coefficients(100)[:5]
+    g = c.gauge_load(torch.from_numpy(U).float().cuda(), dims, 4, 12, -1)
+    vs = [inputs.round_to_f32(inputs.spinor_field(dims, 0, 30 + i)) for i in range(2)]
+    batch = torch.cat([c.spinor_pack(torch.from_numpy(v).float().cuda(), dims) for v in vs])
+    y = torch.empty_like(batch)
+    c.set_workspace(None)
+    c.ensure_workspace(2 * batch.numel() * 4)
+    c.cheb_apply_multi(y, batch, 2, g, kappa, coeff, scale)
+    n = batch.numel() // 2
+    for i, v in enumerate(vs):
+        want = orc.cheb(v, U, dims, kappa, coeff, scale)
+        got = c.spinor_unpack(y[i * n:(i + 1) * n].contiguous(), dims).cpu().numpy()
+        assert relerr(got, want) <= 2e-6
+    c.set_workspace(None)
