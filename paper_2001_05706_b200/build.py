@@ -51,7 +51,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         src = os.path.join(CSRC, u + ".cu")
         obj = os.path.join(OBJ, u + ".o")
         if force or _stale(obj, [src] + deps):
-            cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+            extra = os.environ.get("QCD_NVCC_EXTRA", "").split()
+            cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
             r = subprocess.run(cmd, capture_output=True, text=True)
             if r.returncode != 0:
                 raise RuntimeError("nvcc failed for %s:\n%s\n%s" % (u, r.stdout, r.stderr))

@@ -253,8 +253,15 @@ __device__ __forceinline__ void hop_site(T (&acc)[24], const Links& L, const T* 
     hop_dir<T, 3, -1, SB>(acc, L, in, Vh, cb, n.tm, n.sgn_tm);
 }
 
+#ifndef HOP_MINBLOCKS_F32
+#define HOP_MINBLOCKS_F32 4
+#endif
+#ifndef HOP_MINBLOCKS_F64
+#define HOP_MINBLOCKS_F64 2
+#endif
+
 template <typename T, int RECON, int DAG, int MODE>
-__global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_kernel(const HopArgs<T> A)
+__global__ void __launch_bounds__(128, (sizeof(T) == 4 ? HOP_MINBLOCKS_F32 : HOP_MINBLOCKS_F64)) hop_kernel(const HopArgs<T> A)
 {
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= A.geo.Vh) return;
