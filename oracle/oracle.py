@@ -41,7 +41,7 @@ def lib():
         _lib = C.CDLL(_SO)
         _lib.orc_num_threads.restype = C.c_int
         _lib.orc_invert_12.restype = C.c_int
-        for n in ("orc_apply_M", "orc_cg", "orc_cg_mixed", "orc_cheb"):
+        for n in ("orc_apply_M", "orc_cg", "orc_cg_mixed", "orc_cheb", "orc_cg_multishift"):
             getattr(_lib, n).restype = C.c_int
     return _lib
 
@@ -197,6 +197,26 @@ def cg_mixed(b, U, dims, kappa, tol, maxiter, A=None, Ainv=None, tb=-1, mode=2, 
         raise MemoryError
     return y, dict(iters=int(st[0]), r_iter=st[1], r_true=st[2], converged=bool(st[3]),
                    breakdown=bool(st[4]), reliable_updates=int(st[5]))
+
+
+def cg_multishift(b, U, dims, kappa, shifts, tol, maxiter, A=None, Ainv=None, tb=-1, mode=2):
+    """Multi-shift CG: (M^dag M + shifts[i]) x_i = b with one N apply per iteration
+    (SURVEY.md 8(f).3).  shifts ascending, >= 0.  Returns ([x_i], stats dict)."""
+    b = _f64(b); U = _f64(U)
+    sh = np.ascontiguousarray(shifts, dtype=np.float64)
+    ns = len(sh)
+    X, Y, Z, T = (int(d) for d in dims)
+    x = np.empty((ns, T, Z, Y, X, 4, 3, 2), dtype=np.float64)
+    st = np.zeros(8, dtype=np.float64)
+    rt = np.zeros(ns, dtype=np.float64)
+    rc = lib().orc_cg_multishift(_p(x), _p(b), _p(U), None if A is None else _p(_f64(A)),
+                                 None if Ainv is None else _p(_f64(Ainv)), _dims(dims), C.c_double(kappa),
+                                 C.c_int(tb), C.c_int(mode), _p(sh), C.c_int(ns), C.c_double(tol),
+                                 C.c_int(maxiter), _p(st), _p(rt))
+    if rc:
+        raise MemoryError
+    return [x[i] for i in range(ns)], dict(iters=int(st[0]), r_iter=st[1], converged=bool(st[3]),
+                                           breakdown=bool(st[4]), r_true=rt.copy())
 
 
 def apply_HW(psi, U, dims, kappa, tb=-1) -> np.ndarray:

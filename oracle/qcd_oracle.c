@@ -445,6 +445,94 @@ int orc_cg_mixed(double *y_, const double *b_, const double *Uhi, const double *
     return 0;
 }
 
+/* ---- multi-shift CG (PAPER.md:169 ref. [5], the GWU-code solver family) ---
+ * Solves (N + sigma_i) x_i = b, i = 0..ns-1, N = M^dag M, shifts ascending, sigma_i >= 0,
+ * with ONE application of N per iteration.  Base system: CG on N + sigma_0 exactly as orc_cg
+ * (reading O6); the shifted systems ride on the collinearity of the residuals,
+ * r_i^n = zeta_i^n r^n (B. Jegerlehner, hep-lat/9612014, in the alpha/beta notation of O6):
+ *   s_i = sigma_i - sigma_0,  zeta_i^{-1} = zeta_i^0 = 1,  alpha_{-1} = 1,  beta_{-1} = 0
+ *   q = (N + sigma_0) p_0 ; alpha_n = rho_n / Re<p_0, q>
+ *   zeta_i^{n+1} = zeta_i^n zeta_i^{n-1} alpha_{n-1}
+ *                  / ( alpha_n beta_{n-1} (zeta_i^{n-1} - zeta_i^n) + zeta_i^{n-1} alpha_{n-1} (1 + s_i alpha_n) )
+ *   x_i += alpha_n (zeta_i^{n+1}/zeta_i^n) p_i ;  r -= alpha_n q ; rho_{n+1} = |r|^2
+ *   stop when |r| <= tol |b|  (the smallest shift converges last: |zeta_i| <= 1)
+ *   beta_n = rho_{n+1}/rho_n ;  p_i = zeta_i^{n+1} r + beta_n (zeta_i^{n+1}/zeta_i^n)^2 p_i
+ * x: ns consecutive fields.  stats[0]=iters, [1]=iterated |r|/|b|, [3]=converged, [4]=breakdown;
+ * rtrue[i] = |b - (N + sigma_i) x_i| / |b| recomputed from scratch.
+ */
+int orc_cg_multishift(double *x_, const double *b_, const double *U, const double *A, const double *Ainv,
+                      const int *dims, double kappa, int tb, int mode, const double *sigma, int ns,
+                      double tol, int maxiter, double *stats, double *rtrue)
+{
+    const long n = (long)dims[0] * dims[1] * dims[2] * dims[3] * 12;
+    orc_op_f64 op;
+    fill_op64(&op, U, A, Ainv, dims, kappa, tb, mode);
+    zc *x = (zc *)x_;
+    const zc *b = (const zc *)b_;
+    zc *r = malloc(n * sizeof(zc)), *q = malloc(n * sizeof(zc)), *tmp = malloc(n * sizeof(zc));
+    zc *t1 = malloc(n * sizeof(zc)), *t2 = malloc(n * sizeof(zc)), *p = malloc((size_t)ns * n * sizeof(zc));
+    double *zm = malloc(ns * sizeof(double)), *z0 = malloc(ns * sizeof(double)), *zp = malloc(ns * sizeof(double));
+    if (!r || !q || !tmp || !t1 || !t2 || !p || !zm || !z0 || !zp) {
+        free(r); free(q); free(tmp); free(t1); free(t2); free(p); free(zm); free(z0); free(zp);
+        return -1;
+    }
+    for (long i = 0; i < n; i++) r[i] = b[i];
+    for (int s = 0; s < ns; s++) {
+        zm[s] = z0[s] = 1.0;
+        for (long i = 0; i < n; i++) { x[s * n + i] = 0; p[s * n + i] = b[i]; }
+    }
+    const double bnorm = sqrt(norm2_f64(b, n));
+    double rho = bnorm * bnorm, alpha_old = 1.0, beta_old = 0.0, rnorm = bnorm;
+    int k = 0, conv = (bnorm == 0.0), brk = 0;
+    while (!conv && k < maxiter) {
+        k++;
+        apply_N_f64(q, p, &op, tmp, t1, t2);
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < n; i++) q[i] += sigma[0] * p[i];
+        const double pq = redot_f64(p, q, n);
+        if (!(pq > 0.0)) { brk = 1; break; }
+        const double alpha = rho / pq;
+        for (int s = 0; s < ns; s++) {
+            const double sh = sigma[s] - sigma[0];
+            zp[s] = z0[s] * zm[s] * alpha_old /
+                    (alpha * beta_old * (zm[s] - z0[s]) + zm[s] * alpha_old * (1.0 + sh * alpha));
+            const double as = alpha * zp[s] / z0[s];
+            zc *xs = x + (long)s * n, *ps = p + (long)s * n;
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; i++) xs[i] += as * ps[i];
+        }
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < n; i++) r[i] -= alpha * q[i];
+        const double rho2 = norm2_f64(r, n);
+        rnorm = sqrt(rho2);
+        if (rnorm <= tol * bnorm) { conv = 1; break; }
+        const double beta = rho2 / rho;
+        for (int s = 0; s < ns; s++) {
+            const double ratio = zp[s] / z0[s], bs = beta * ratio * ratio, zs = zp[s];
+            zc *ps = p + (long)s * n;
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; i++) ps[i] = zs * r[i] + bs * ps[i];
+            zm[s] = z0[s];
+            z0[s] = zp[s];
+        }
+        rho = rho2; alpha_old = alpha; beta_old = beta;
+    }
+    for (int s = 0; s < ns; s++) {
+        const zc *xs = x + (long)s * n;
+        apply_N_f64(q, xs, &op, tmp, t1, t2);
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < n; i++) q[i] = b[i] - q[i] - sigma[s] * xs[i];
+        rtrue[s] = bnorm > 0 ? sqrt(norm2_f64(q, n)) / bnorm : 0.0;
+    }
+    stats[0] = k;
+    stats[1] = bnorm > 0 ? rnorm / bnorm : 0.0;
+    stats[2] = rtrue[0];
+    stats[3] = conv;
+    stats[4] = brk;
+    free(r); free(q); free(tmp); free(t1); free(t2); free(p); free(zm); free(z0); free(zp);
+    return 0;
+}
+
 /* ---- Chebyshev polynomial of H_W = gamma5 D_W, reading O8 / S16 -------------
  *   X = H_W/scale;  T_0 v = v, T_1 v = X v, T_{k+1} v = 2 X T_k v - T_{k-1} v
  *   y = sum_{k=0}^{degree} coeff[k] T_k v        (forward three-term recurrence)

@@ -460,3 +460,45 @@ def test_p11_mixed_cg_matches_pure_cg():
         assert abs(sm["iters"] - st["iters"]) <= max(6, 0.08 * st["iters"])
         assert sm["reliable_updates"] >= 3
         assert relerr(y, x) < 1e-8
+
+
+# ---- multi-shift CG ----------------------------------------------------
+def test_multishift_cg_matches_dense_shifted_solves_on_2to4():
+    """Brute force: (D^dag D + sigma_i) x_i = b by LU on the 192 x 192 dense matrix."""
+    dims, kappa = (2, 2, 2, 2), 0.135
+    U = inputs.gauge_field(dims, 0.5, 0)
+    D = dense_matrix(lambda v: orc.apply_M(v, U, dims, kappa), dims)
+    N = D.conj().T @ D
+    b = inputs.spinor_field(dims, 0, 1)
+    shifts = [0.0, 0.01, 0.1, 1.0, 10.0]
+    xs, st = orc.cg_multishift(b, U, dims, kappa, shifts, 1e-12, 1000)
+    assert st["converged"] and not st["breakdown"]
+    bc = cplx(b).reshape(-1)
+    for x, sg in zip(xs, shifts):
+        want = np.linalg.solve(N + sg * np.eye(N.shape[0]), bc)
+        assert relerr(cplx(x).reshape(-1), want) < 1e-10
+    assert st["r_true"].max() < 2e-12
+
+
+def test_multishift_cg_reduces_to_plain_cg_and_each_shift_to_its_own_cg():
+    dims, kappa = (4, 4, 4, 8), 0.135
+    U = inputs.gauge_field(dims, 0.5, 0)
+    _, A, Ainv = clover_fields(U, dims, kappa, 1.0)
+    b = inputs.spinor_field(dims, 0, 1)
+    x_ref, st_ref = orc.cg(b, U, dims, kappa, 1e-10, 2000, A, Ainv)
+    # one shift equal to zero: the same iteration, iterate for iterate
+    xs, st = orc.cg_multishift(b, U, dims, kappa, [0.0], 1e-10, 2000, A, Ainv)
+    assert st["iters"] == st_ref["iters"]
+    assert relerr(xs[0], x_ref) < 1e-13
+    # several shifts: the unshifted member is unchanged, every member meets its residual,
+    # and the shifted residuals obey |b - (N + s) x_s| <= |b - N x_0| (|zeta| <= 1)
+    shifts = [0.0, 0.05, 0.5, 5.0]
+    xs, st = orc.cg_multishift(b, U, dims, kappa, shifts, 1e-10, 2000, A, Ainv)
+    assert st["iters"] == st_ref["iters"]
+    assert relerr(xs[0], x_ref) < 1e-12
+    assert (st["r_true"] < 1.5e-10).all()
+    assert (st["r_true"][1:] <= st["r_true"][0] * 1.01).all()
+    # non-zero base shift: compare with a dense-free identity, (N + s0) x = b  <=>  residual check
+    xs2, st2 = orc.cg_multishift(b, U, dims, kappa, [0.5, 5.0], 1e-10, 2000, A, Ainv)
+    assert relerr(xs2[0], xs[2]) < 1e-9 and relerr(xs2[1], xs[3]) < 1e-9
+    assert st2["iters"] < st["iters"]
