@@ -301,6 +301,15 @@ def solver_table(c, w):
         out[name] = {"seconds": round(st.seconds, 5), "iters": st.iters, "reliable_updates": st.reliable_updates,
                      "r_true": st.r_true, "rc": rc, "GFLOP/s": round(st.flops / st.seconds * 1e-9, 1),
                      "ms_per_iter": round(st.seconds / max(st.iters, 1) * 1e3, 4)}
+    # multi-shift CG: 4 shifted systems for the price of one N apply per iteration
+    shifts = [0.0, 0.01, 0.1, 1.0]
+    xs = torch.empty(len(shifts) * h, dtype=b.dtype, device="cuda")
+    c.set_operator(w["g64"], None, w["c64"], None, KAPPA, CSW, 0)
+    c.ensure_workspace((4 + len(shifts)) * h * 8)
+    c.cg_multishift(xs, b, shifts, 1e-10, 5000)
+    rc, st, rts = c.cg_multishift(xs, b, shifts, 1e-10, 5000)
+    out["multishift_cg_fp64_18 (4 shifts)"] = {"seconds": round(st.seconds, 5), "iters": st.iters, "rc": rc, "shifts": shifts,
+                                               "r_true_max": max(rts), "ms_per_iter": round(st.seconds / max(st.iters, 1) * 1e3, 4)}
     return out
 
 

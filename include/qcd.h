@@ -182,6 +182,14 @@ int qcd_set_operator(qcd_ctx* ctx, const qcd_gauge* g_hi, const qcd_gauge* g_lo,
 int qcd_cg_solve(void* x, const void* b, double tol, int maxiter);
 int qcd_cg_solve_ex(qcd_ctx* ctx, void* x, const void* b, double tol, int maxiter,
                     qcd_stats* stats);
+/* Multi-shift CG (PAPER.md:169 ref. [5]): solves (M^dag M + shifts[i]) x_i = b
+ * for nshift <= 16 strictly ascending shifts >= 0 with ONE application of M^dag M per
+ * iteration (B. Jegerlehner, hep-lat/9612014).  x: nshift consecutive fields (out), b: one
+ * field, both in the precision of the (pure-precision) operator of qcd_set_operator.
+ * shifts, r_true: HOST arrays; r_true (may be NULL) receives |b - (N + s_i) x_i| / |b|.
+ * Stops when the base (smallest-shift) residual meets tol.  Workspace: (4 + nshift) fields. */
+int qcd_cg_multishift(qcd_ctx* ctx, void* x, const void* b, const double* shifts, int nshift,
+                      double tol, int maxiter, qcd_stats* stats, double* r_true);
 /* out = M in (flags & QCD_DAGGER: M^dag in) for the operator of qcd_set_operator, in
  * the high precision. */
 int qcd_apply_operator(qcd_ctx* ctx, void* out, const void* in, int flags);

@@ -189,6 +189,62 @@ template <int HI_TO_LO> __global__ void __launch_bounds__(BLAS_THREADS) convert_
     }
 }
 
+/* ---- multi-shift CG updates: one pass over all shifted systems ------- */
+template <typename T>
+__global__ void __launch_bounds__(BLAS_THREADS) multishift_x_kernel(MultiShiftCoef cf, T* x, const T* p, size_t fstride_vec, const T* q, T* r,
+                                    size_t nvec, double* partial, unsigned int* ticket, double* out)
+{
+    typedef typename Vec<T>::type V;
+    const V* qv = reinterpret_cast<const V*>(q);
+    V* rv = reinterpret_cast<V*>(r);
+    const T alpha = (T)cf.alpha;
+    double s = 0.0;
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
+        T qs[Vec<T>::reals], rs[Vec<T>::reals];
+        vec_get(qv[i], qs);
+        vec_get(rv[i], rs);
+#pragma unroll
+        for (int k = 0; k < Vec<T>::reals; k++) {
+            rs[k] -= alpha * qs[k];
+            s += (double)rs[k] * (double)rs[k];
+        }
+        rv[i] = vec_make(rs);
+        for (int j = 0; j < cf.ns; j++) {
+            V* xv = reinterpret_cast<V*>(x) + (size_t)j * fstride_vec;
+            const V* pv = reinterpret_cast<const V*>(p) + (size_t)j * fstride_vec;
+            T xs[Vec<T>::reals], ps[Vec<T>::reals];
+            vec_get(xv[i], xs);
+            vec_get(pv[i], ps);
+            const T a = (T)cf.c[j];
+#pragma unroll
+            for (int k = 0; k < Vec<T>::reals; k++) xs[k] += a * ps[k];
+            xv[i] = vec_make(xs);
+        }
+    }
+    double tot;
+    if (grid_sum(s, partial, ticket, &tot)) *out = tot;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(BLAS_THREADS) multishift_p_kernel(MultiShiftCoef zeta, MultiShiftCoef beta, T* p, size_t fstride_vec, const T* r, size_t nvec)
+{
+    typedef typename Vec<T>::type V;
+    const V* rv = reinterpret_cast<const V*>(r);
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
+        T rs[Vec<T>::reals];
+        vec_get(rv[i], rs);
+        for (int j = 0; j < zeta.ns; j++) {
+            V* pv = reinterpret_cast<V*>(p) + (size_t)j * fstride_vec;
+            T ps[Vec<T>::reals];
+            vec_get(pv[i], ps);
+            const T z = (T)zeta.c[j], b = (T)beta.c[j];
+#pragma unroll
+            for (int k = 0; k < Vec<T>::reals; k++) ps[k] = z * rs[k] + b * ps[k];
+            pv[i] = vec_make(ps);
+        }
+    }
+}
+
 int grid_for(const qcd_ctx* ctx, size_t nvec)
 {
     size_t b = (nvec + BLAS_THREADS - 1) / BLAS_THREADS;
@@ -298,4 +354,31 @@ int blas_copy(qcd_ctx* ctx, void* dst, const void* src, size_t bytes)
     cudaError_t e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, ctx->stream);
     if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "memcpy: %s", cudaGetErrorString(e));
     return QCD_OK;
+}
+
+int blas_multishift_x(qcd_ctx* ctx, const MultiShiftCoef& cf, void* x, const void* p, const void* q, void* r, size_t nreal, int prec,
+                      double* d_out)
+{
+    if (prec == 4) {
+        const size_t nv = nreal / 4;
+        multishift_x_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(cf, (float*)x, (const float*)p, nv, (const float*)q, (float*)r, nv,
+                                                                                      ctx->d_partial, ctx->d_ticket, d_out);
+    } else {
+        const size_t nv = nreal / 2;
+        multishift_x_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(cf, (double*)x, (const double*)p, nv, (const double*)q, (double*)r,
+                                                                                       nv, ctx->d_partial, ctx->d_ticket, d_out);
+    }
+    return check_launch(ctx, "multishift_x");
+}
+
+int blas_multishift_p(qcd_ctx* ctx, const MultiShiftCoef& zeta, const MultiShiftCoef& beta, void* p, const void* r, size_t nreal, int prec)
+{
+    if (prec == 4) {
+        const size_t nv = nreal / 4;
+        multishift_p_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(zeta, beta, (float*)p, nv, (const float*)r, nv);
+    } else {
+        const size_t nv = nreal / 2;
+        multishift_p_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(zeta, beta, (double*)p, nv, (const double*)r, nv);
+    }
+    return check_launch(ctx, "multishift_p");
 }

@@ -140,6 +140,19 @@ int blas_residual_hi(qcd_ctx*, void* r_hi, void* r_lo, const void* b, const void
                      size_t Vh, double* d_out);
 /* internal-layout spinor blocks of Vh sites each (nreal = nblocks*24*Vh), layout-aware */
 int blas_convert(qcd_ctx*, void* dst, int pdst, const void* src, int psrc, size_t nreal, size_t Vh);
+/* multi-shift CG: ns consecutive fields of nreal reals in x and p */
+enum { QCD_MAX_SHIFTS = 16 };
+struct MultiShiftCoef {
+    int ns;
+    double alpha;
+    double c[QCD_MAX_SHIFTS];
+};
+/* r -= alpha q ; *d_out = |r|^2 ; x_j += c[j] p_j */
+int blas_multishift_x(qcd_ctx*, const MultiShiftCoef& cf, void* x, const void* p, const void* q, void* r, size_t nreal,
+                      int prec, double* d_out);
+/* p_j = zeta.c[j] r + beta.c[j] p_j */
+int blas_multishift_p(qcd_ctx*, const MultiShiftCoef& zeta, const MultiShiftCoef& beta, void* p, const void* r, size_t nreal,
+                      int prec);
 int blas_zero(qcd_ctx*, void* x, size_t bytes);
 int blas_copy(qcd_ctx*, void* dst, const void* src, size_t bytes);
 

@@ -278,6 +278,108 @@ int qcd_cg_solve(void* x, const void* b, double tol, int maxiter)
     return qcd_cg_solve_ex(g_last_ctx, x, b, tol, maxiter, nullptr);
 }
 
+int qcd_cg_multishift(qcd_ctx* ctx, void* x, const void* b, const double* shifts, int nshift, double tol, int maxiter,
+                      qcd_stats* stats, double* r_true)
+{
+    QCD_REQUIRE(ctx && ctx->op_set, "cg_multishift: no operator set (qcd_set_operator)");
+    QCD_REQUIRE(!ctx->g_lo, "cg_multishift: pure-precision operator only");
+    QCD_REQUIRE(x && b && shifts && (((uintptr_t)x | (uintptr_t)b) & 15u) == 0, "cg_multishift: bad pointer");
+    QCD_REQUIRE(nshift >= 1 && nshift <= QCD_MAX_SHIFTS, "cg_multishift: 1 <= nshift <= %d", (int)QCD_MAX_SHIFTS);
+    QCD_REQUIRE(tol > 0.0 && maxiter >= 0, "cg_multishift: tol must be > 0 and maxiter >= 0");
+    for (int i = 0; i < nshift; i++)
+        QCD_REQUIRE(shifts[i] >= 0.0 && (i == 0 || shifts[i] > shifts[i - 1]), "cg_multishift: shifts must be >= 0 and strictly ascending");
+    const Op o = make_op(ctx, ctx->g_hi, ctx->c_hi);
+    const int P = o.g->precision;
+    const size_t need = (size_t)(4 + nshift) * o.bytes;
+    QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= need, "cg_multishift: workspace too small (need %zu bytes)", need);
+    {
+        const uintptr_t a0 = (uintptr_t)x, a1 = (uintptr_t)b;
+        QCD_REQUIRE(a0 + nshift * o.bytes <= a1 || a1 + o.bytes <= a0, "cg_multishift: x and b alias");
+    }
+    char* w = (char*)ctx->ws;
+    void *r = w, *q = w + o.bytes, *t = w + 2 * o.bytes, *tmp = w + 3 * o.bytes;
+    char* p = w + 4 * o.bytes;
+    double* d = ctx->d_scalar;
+    double* h = ctx->h_scalar;
+    cudaEvent_t e0, e1;
+    QCD_CHECK_CUDA(cudaEventCreate(&e0));
+    QCD_CHECK_CUDA(cudaEventCreate(&e1));
+    QCD_CHECK_CUDA(cudaEventRecord(e0, ctx->stream));
+
+    RC(blas_zero(ctx, x, nshift * o.bytes));
+    RC(blas_copy(ctx, r, b, o.bytes));
+    for (int s = 0; s < nshift; s++) RC(blas_copy(ctx, p + s * o.bytes, b, o.bytes));
+    RC(blas_norm2(ctx, b, o.nreal, P, d + S_RHO_A));
+    RC(fetch(ctx, S_RHO_A, 1));
+    const double bnorm = sqrt(h[S_RHO_A]);
+    double rho = h[S_RHO_A], alpha_old = 1.0, beta_old = 0.0, rnorm = bnorm;
+    double zm[QCD_MAX_SHIFTS], z0[QCD_MAX_SHIFTS], zp[QCD_MAX_SHIFTS];
+    for (int s = 0; s < nshift; s++) zm[s] = z0[s] = 1.0;
+    int k = 0, conv = (bnorm == 0.0), brk = 0;
+    while (!conv && k < maxiter) {
+        k++;
+        RC(apply_N(o, q, p, t, tmp));
+        if (shifts[0] != 0.0) RC(blas_axpby(ctx, host_scalar(shifts[0]), p, host_scalar(1.0), q, o.nreal, P));
+        RC(blas_redot(ctx, p, q, o.nreal, P, d + S_PQ));
+        RC(fetch(ctx, S_PQ, 1));
+        const double pq = h[S_PQ];
+        if (!(pq > 0.0)) { brk = 1; break; }
+        const double alpha = rho / pq;
+        MultiShiftCoef cx;
+        cx.ns = nshift; cx.alpha = alpha;
+        for (int s = 0; s < nshift; s++) {
+            const double sh = shifts[s] - shifts[0];
+            zp[s] = z0[s] * zm[s] * alpha_old / (alpha * beta_old * (zm[s] - z0[s]) + zm[s] * alpha_old * (1.0 + sh * alpha));
+            cx.c[s] = alpha * zp[s] / z0[s];
+        }
+        RC(blas_multishift_x(ctx, cx, x, p, q, r, o.nreal, P, d + S_RHO_B));
+        RC(fetch(ctx, S_RHO_B, 1));
+        const double rho2 = h[S_RHO_B];
+        rnorm = sqrt(rho2);
+        if (rnorm <= tol * bnorm) { conv = 1; break; }
+        const double beta = rho2 / rho;
+        MultiShiftCoef cz, cb;
+        cz.ns = cb.ns = nshift; cz.alpha = cb.alpha = 0.0;
+        for (int s = 0; s < nshift; s++) {
+            const double ratio = zp[s] / z0[s];
+            cz.c[s] = zp[s];
+            cb.c[s] = beta * ratio * ratio;
+            zm[s] = z0[s];
+            z0[s] = zp[s];
+        }
+        RC(blas_multishift_p(ctx, cz, cb, p, r, o.nreal, P));
+        rho = rho2; alpha_old = alpha; beta_old = beta;
+    }
+    cudaEventRecord(e1, ctx->stream);
+    cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    double rt0 = 0.0;
+    for (int s = 0; s < nshift && (r_true || s == 0); s++) {
+        const char* xs = (const char*)x + s * o.bytes;
+        RC(apply_N(o, q, xs, t, tmp));
+        if (shifts[s] != 0.0) RC(blas_axpby(ctx, host_scalar(shifts[s]), xs, host_scalar(1.0), q, o.nreal, P));
+        RC(blas_axpby(ctx, host_scalar(1.0), b, host_scalar(-1.0), q, o.nreal, P));
+        RC(blas_norm2(ctx, q, o.nreal, P, d + S_AUX));
+        RC(fetch(ctx, S_AUX, 1));
+        const double rt = bnorm > 0 ? sqrt(h[S_AUX]) / bnorm : 0.0;
+        if (r_true) r_true[s] = rt;
+        if (s == 0) rt0 = rt;
+    }
+    if (stats) {
+        memset(stats, 0, sizeof(*stats));
+        stats->iters = k; stats->converged = conv; stats->breakdown = brk;
+        stats->r_iter = bnorm > 0 ? rnorm / bnorm : 0.0;
+        stats->r_true = rt0;
+        stats->seconds = ms * 1e-3;
+        stats->flops = 2.0 * hop_flops_per_apply_M(o) * k;
+    }
+    if (brk) return qcd_set_error(QCD_EBREAKDOWN, "cg_multishift: <p,(N+s)p> <= 0 or NaN at iteration %d", k);
+    return conv ? QCD_OK : QCD_NOCONV;
+}
+
 int qcd_cheb_apply_multi(qcd_ctx* ctx, void* y, const void* v, int nvec, const qcd_gauge* g, double kappa, const double* coeff,
                          int degree, double scale)
 {

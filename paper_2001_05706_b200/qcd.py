@@ -70,6 +70,7 @@ SIGNATURES = {
     "qcd_set_operator": (_i, [_vp, _vp, _vp, _vp, _vp, _d, _d, _i, _d]),
     "qcd_cg_solve": (_i, [_vp, _vp, _d, _i]),
     "qcd_cg_solve_ex": (_i, [_vp, _vp, _vp, _d, _i, C.POINTER(Stats)]),
+    "qcd_cg_multishift": (_i, [_vp, _vp, _vp, C.POINTER(_d), _i, _d, _i, C.POINTER(Stats), C.POINTER(_d)]),
     "qcd_apply_operator": (_i, [_vp, _vp, _vp, _i]),
     "qcd_cheb_apply": (_i, [_vp, _vp, _vp, _vp, _d, C.POINTER(_d), _i, _d]),
     "qcd_cheb_apply_multi": (_i, [_vp, _vp, _vp, _i, _vp, _d, C.POINTER(_d), _i, _d]),
@@ -265,6 +266,15 @@ class Context:
         st = Stats()
         rc = _check(lib().qcd_cg_solve_ex(self.h, _ptr(x), _ptr(b), tol, maxiter, C.byref(st)), soft=True)
         return rc, st
+
+    def cg_multishift(self, x, b, shifts, tol: float, maxiter: int):
+        """x: len(shifts) consecutive fields.  Returns (return code, Stats, [r_true_i])."""
+        ns = len(shifts)
+        sh = (_d * ns)(*[float(v) for v in shifts])
+        rt = (_d * ns)()
+        st = Stats()
+        rc = _check(lib().qcd_cg_multishift(self.h, _ptr(x), _ptr(b), sh, ns, tol, maxiter, C.byref(st), rt), soft=True)
+        return rc, st, [rt[i] for i in range(ns)]
 
     def cheb_apply(self, y, v, gauge: "Gauge", kappa: float, coeff, scale: float):
         n = len(coeff)

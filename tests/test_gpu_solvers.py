@@ -204,3 +204,55 @@ def test_chebyshev_multi_rhs_matches_oracle(precision, recon, dims):
     y1 = torch.empty_like(batch[:n])
     c.cheb_apply(y1, batch[:n].contiguous(), g, kappa, coeff, scale)
     assert relerr(y1.cpu().numpy(), y[:n].cpu().numpy()) <= (1e-6 if precision == 4 else 1e-14)
+
+
+@pytest.mark.parametrize("mode,csw,precision", [(2, 0.0, 8), (0, 1.0, 8), (0, 1.0, 4)])
+def test_multishift_cg_matches_oracle(mode, csw, precision):
+    """(N + sigma_i) x_i = b for all shifts with one N apply per iteration."""
+    c = ctx()
+    dims, kappa = (8, 8, 8, 16), 0.135
+    tol = 1e-10 if precision == 8 else 1e-5
+    shifts = [0.0, 0.01, 0.1, 1.0] if mode == 0 else [0.02, 0.3, 3.0]
+    U, g, cl, A, Ainv = setup_operator(c, dims, kappa, csw, precision, 18)
+    if precision == 4 and A is not None:
+        A, Ainv = inputs.round_to_f32(A), inputs.round_to_f32(Ainv)
+    b = inputs.spinor_field(dims, 0, 1)
+    if precision == 4:
+        b = inputs.round_to_f32(b)
+    if mode != 2:
+        b = b * (parity_mask(dims) == mode)
+    xs_ref, st_ref = orc.cg_multishift(b, U, dims, kappa, shifts, tol, 5000, A, Ainv, -1, mode)
+    pb = pack(c, b, dims, precision)
+    n = pb.numel() if mode == 2 else pb.numel() // 2
+    src = pb if mode == 2 else blocks(pb)[mode].clone()
+    x = torch.empty(len(shifts) * n, dtype=pb.dtype, device="cuda")
+    c.ensure_workspace((4 + len(shifts)) * n * precision)
+    c.set_operator(g, None, cl, None, kappa, csw, mode)
+    rc, st, rts = c.cg_multishift(x, src, shifts, tol, 5000)
+    assert rc == 0 and st.converged == 1
+    assert abs(st.iters - st_ref["iters"]) <= 2
+    assert max(rts) < (1.5 * tol if precision == 8 else 5 * tol)
+    for i in range(len(shifts)):
+        xi = x[i * n:(i + 1) * n]
+        if mode == 2:
+            got = unpack(c, xi.contiguous(), dims)
+        else:
+            full = torch.zeros_like(pb)
+            blocks(full)[mode].copy_(xi)
+            got = unpack(c, full, dims)
+        assert relerr(got, xs_ref[i]) <= (1e-8 if precision == 8 else 1e-3)
+
+
+def test_multishift_argument_errors():
+    from paper_2001_05706_b200 import qcd
+    c = ctx()
+    dims, kappa = (4, 4, 4, 4), 0.125
+    U, g, cl, A, Ainv = setup_operator(c, dims, kappa, 0.0, 8, 18)
+    c.set_operator(g, None, None, None, kappa, 0.0, 2)
+    b = torch.randn(4 ** 4 * 24, device="cuda", dtype=torch.float64)
+    x = torch.empty(2 * b.numel(), device="cuda", dtype=torch.float64)
+    c.ensure_workspace(6 * b.numel() * 8)
+    for bad in ([0.1, 0.1], [0.2, 0.1], [-0.1, 0.1]):
+        with pytest.raises(qcd.QcdError) as e:
+            c.cg_multishift(x, b, bad, 1e-10, 10)
+        assert e.value.code == qcd.EINVAL
