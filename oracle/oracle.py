@@ -41,7 +41,8 @@ def lib():
         _lib = C.CDLL(_SO)
         _lib.orc_num_threads.restype = C.c_int
         _lib.orc_invert_12.restype = C.c_int
-        for n in ("orc_apply_M", "orc_cg", "orc_cg_mixed", "orc_cheb", "orc_cg_multishift"):
+        for n in ("orc_apply_M", "orc_cg", "orc_cg_mixed", "orc_cheb", "orc_cg_multishift", "orc_apply_M_q16",
+                  "orc_apply_N_q16"):
             getattr(_lib, n).restype = C.c_int
     return _lib
 
@@ -179,20 +180,81 @@ def cg(b, U, dims, kappa, tol, maxiter, A=None, Ainv=None, tb=-1, mode=2):
                    breakdown=bool(st[4]))
 
 
-def cg_mixed(b, U, dims, kappa, tol, maxiter, A=None, Ainv=None, tb=-1, mode=2, delta=0.1):
+def q16_codes(v):
+    """(int16 codes [n][24], fp32 norms [n]) of the 16-bit spinor format (reading H1)."""
+    v = np.ascontiguousarray(v, dtype=np.float32).reshape(-1, 24)
+    codes = np.empty(v.shape, dtype=np.int16)
+    norms = np.empty(len(v), dtype=np.float32)
+    lib().orc_q16_codes(_p(v), _p(codes), _p(norms), C.c_long(len(v)))
+    return codes, norms
+
+
+def q16_spinor(v):
+    """Spinor stored in 16 bits and read back (fp32 array, same shape)."""
+    out = np.array(v, dtype=np.float32, order="C")
+    lib().orc_q16_spinor(_p(out), C.c_long(out.size // 24))
+    return out
+
+
+def q16_links(U):
+    out = np.array(U, dtype=np.float32, order="C")
+    lib().orc_q16_links(_p(out), C.c_long(out.size // 18))
+    return out
+
+
+def q16_clover(A):
+    out = np.array(A, dtype=np.float32, order="C")
+    lib().orc_q16_clover(_p(out), C.c_long(out.size // 288))
+    return out
+
+
+def apply_M_q16(psi_q, Uq, dims, kappa, Aq=None, Ainvq=None, tb=-1, mode=2, dagger=False, store_out=False):
+    """M (or M^dag) with 16-bit storage of links, clover and the even-odd intermediate; psi_q,
+    Uq, Aq, Ainvq are stored-and-read-back fp32 fields (q16_*).  Returns fp32."""
+    psi_q = np.ascontiguousarray(psi_q, dtype=np.float32)
+    out = np.empty_like(psi_q)
+    rc = lib().orc_apply_M_q16(_p(out), _p(psi_q), _p(np.ascontiguousarray(Uq, dtype=np.float32)),
+                               None if Aq is None else _p(np.ascontiguousarray(Aq, dtype=np.float32)),
+                               None if Ainvq is None else _p(np.ascontiguousarray(Ainvq, dtype=np.float32)),
+                               _dims(dims), C.c_double(kappa), C.c_int(tb), C.c_int(mode), C.c_int(int(dagger)),
+                               C.c_int(int(store_out)))
+    if rc:
+        raise MemoryError
+    return out
+
+
+def apply_N_q16(p, Uq, dims, kappa, Aq=None, Ainvq=None, tb=-1, mode=2):
+    """q = M^dag store(M store(p)) with every streamed field in 16 bits; q in fp32."""
+    p = np.ascontiguousarray(p, dtype=np.float32)
+    out = np.empty_like(p)
+    rc = lib().orc_apply_N_q16(_p(out), _p(p), _p(np.ascontiguousarray(Uq, dtype=np.float32)),
+                               None if Aq is None else _p(np.ascontiguousarray(Aq, dtype=np.float32)),
+                               None if Ainvq is None else _p(np.ascontiguousarray(Ainvq, dtype=np.float32)),
+                               _dims(dims), C.c_double(kappa), C.c_int(tb), C.c_int(mode))
+    if rc:
+        raise MemoryError
+    return out
+
+
+def cg_mixed(b, U, dims, kappa, tol, maxiter, A=None, Ainv=None, tb=-1, mode=2, delta=0.1, half=False):
     """Reliable-update fp32/fp64 CG (reading O7).  The fp32 operator uses the
-    fp64 fields rounded to fp32 (reading S15)."""
+    fp64 fields rounded to fp32 (reading S15); with half=True the inner operator streams
+    16-bit fields (reading H1): links, clover and spinors stored in 16 bits."""
     b = _f64(b); U = _f64(U)
     Ulo = np.ascontiguousarray(U, dtype=np.float32)
     Alo = None if A is None else np.ascontiguousarray(A, dtype=np.float32)
     Ailo = None if Ainv is None else np.ascontiguousarray(Ainv, dtype=np.float32)
+    if half:
+        Ulo = q16_links(Ulo)
+        Alo = None if Alo is None else q16_clover(Alo)
+        Ailo = None if Ailo is None else q16_clover(Ailo)
     y = _spinor_like(dims)
     st = np.zeros(8, dtype=np.float64)
     rc = lib().orc_cg_mixed(_p(y), _p(b), _p(U), None if A is None else _p(_f64(A)),
                             None if Ainv is None else _p(_f64(Ainv)), _p(Ulo),
                             None if Alo is None else _p(Alo), None if Ailo is None else _p(Ailo),
                             _dims(dims), C.c_double(kappa), C.c_int(tb), C.c_int(mode),
-                            C.c_double(tol), C.c_int(maxiter), C.c_double(delta), _p(st))
+                            C.c_double(tol), C.c_int(maxiter), C.c_double(delta), C.c_int(int(half)), _p(st))
     if rc:
         raise MemoryError
     return y, dict(iters=int(st[0]), r_iter=st[1], r_true=st[2], converged=bool(st[3]),

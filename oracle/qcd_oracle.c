@@ -357,6 +357,8 @@ int orc_cg(double *x_, const double *b_, const double *U, const double *A, const
     return 0;
 }
 
+static void apply_N_q16(fc *q, const fc *p, const orc_op_f32 *op, fc *tmp, fc *t1, fc *t2, fc *ph);
+
 /* ---- reliable-update mixed-precision CG, reading O7 / S15 (PAPER.md:163 ref [1])
  * Inner vectors x,r,p,q and N in fp32 (Ulo/Alo/Ainvlo = the fp64 fields rounded to
  * fp32 by the caller); y, r_hi and N_hi in fp64; delta = 0.1 by default.
@@ -372,7 +374,7 @@ int orc_cg(double *x_, const double *b_, const double *U, const double *A, const
 int orc_cg_mixed(double *y_, const double *b_, const double *Uhi, const double *Ahi,
                  const double *Ainvhi, const float *Ulo, const float *Alo, const float *Ainvlo,
                  const int *dims, double kappa, int tb, int mode, double tol, int maxiter,
-                 double delta, double *stats)
+                 double delta, int half, double *stats)
 {
     const long n = (long)dims[0] * dims[1] * dims[2] * dims[3] * 12;
     orc_op_f64 ohi;
@@ -385,10 +387,10 @@ int orc_cg_mixed(double *y_, const double *b_, const double *Uhi, const double *
        *h2 = malloc(n * sizeof(zc));
     fc *x = malloc(n * sizeof(fc)), *r = malloc(n * sizeof(fc)), *p = malloc(n * sizeof(fc)),
        *q = malloc(n * sizeof(fc)), *tl = malloc(n * sizeof(fc)), *l1 = malloc(n * sizeof(fc)),
-       *l2 = malloc(n * sizeof(fc));
-    if (!rh || !th || !h1 || !h2 || !x || !r || !p || !q || !tl || !l1 || !l2) {
+       *l2 = malloc(n * sizeof(fc)), *ph = malloc(n * sizeof(fc));
+    if (!rh || !th || !h1 || !h2 || !x || !r || !p || !q || !tl || !l1 || !l2 || !ph) {
         free(rh); free(th); free(h1); free(h2); free(x); free(r); free(p); free(q); free(tl);
-        free(l1); free(l2);
+        free(l1); free(l2); free(ph);
         return -1;
     }
     for (long i = 0; i < n; i++) {
@@ -401,7 +403,9 @@ int orc_cg_mixed(double *y_, const double *b_, const double *Uhi, const double *
     if (bnorm == 0.0) conv = 1;
     while (!conv && k < maxiter) {
         k++;
-        apply_N_f32(q, p, &olo, tl, l1, l2);
+        /* half != 0: the inner operator streams 16-bit fields (reading H1); x, r, p, q stay fp32 */
+        if (half) apply_N_q16(q, p, &olo, tl, l1, l2, ph);
+        else apply_N_f32(q, p, &olo, tl, l1, l2);
         const double pq = redot_f32(p, q, n);
         if (!(pq > 0.0)) { brk = 1; break; }
         const float alpha = (float)(rho / pq);
@@ -441,7 +445,154 @@ int orc_cg_mixed(double *y_, const double *b_, const double *Uhi, const double *
     stats[4] = brk;
     stats[5] = nup;
     free(rh); free(th); free(h1); free(h2); free(x); free(r); free(p); free(q); free(tl);
-    free(l1); free(l2);
+    free(l1); free(l2); free(ph);
+    return 0;
+}
+
+/* ---- 16-bit fixed-point storage for the low-precision operator (
+ * PAPER.md:163 ref. [1], mixed-precision solvers with a 16-bit "half" format) -------------
+ * Reading H1: the paper gives no format; this build's is
+ *   spinor site (24 reals v_k): n = max_k |v_k| (fp32); code_k = rintf(v_k * (32767.0f / n)),
+ *       an int16 (all codes 0 when n = 0); value read back = (float)code_k * (n / 32767.0f).
+ *   link: the 12 reals of rows 0,1 (|u| <= 1): code = rintf(u * 32767.0f) clamped to
+ *       +-32767, read back = (float)code * (1.0f/32767.0f); row 2 = conj(row0 x row1) of the
+ *       values read back (fp32).
+ *   clover site (A or A^-1, Hermitian, 2 chiral 6x6 blocks): n = max |Re|,|Im| over the
+ *       diagonal and lower triangle; codes and read-back as for a spinor site; upper
+ *       triangle = conjugate of the lower one, diagonal real, off-chirality blocks zero.
+ * All fp32, round-to-nearest-even.  The functions below apply "store then read back" in
+ * place, so that the rest of the oracle can keep working on plain float arrays.
+ */
+static inline float q16_code(float v, float scale)
+{
+    float c = rintf(v * scale);
+    if (c > 32767.0f) c = 32767.0f;
+    if (c < -32767.0f) c = -32767.0f;
+    return c;
+}
+void orc_q16_codes(const float *v, short *codes, float *norms, long nsites)
+{
+    for (long s = 0; s < nsites; s++) {
+        float n = 0.0f;
+        for (int k = 0; k < 24; k++) n = fmaxf(n, fabsf(v[s * 24 + k]));
+        norms[s] = n;
+        const float scale = n > 0.0f ? 32767.0f / n : 0.0f;
+        for (int k = 0; k < 24; k++) codes[s * 24 + k] = (short)q16_code(v[s * 24 + k], scale);
+    }
+}
+void orc_q16_spinor(float *v, long nsites)
+{
+#pragma omp parallel for schedule(static)
+    for (long s = 0; s < nsites; s++) {
+        float n = 0.0f;
+        for (int k = 0; k < 24; k++) n = fmaxf(n, fabsf(v[s * 24 + k]));
+        const float scale = n > 0.0f ? 32767.0f / n : 0.0f;
+        const float d = n / 32767.0f;
+        for (int k = 0; k < 24; k++) v[s * 24 + k] = q16_code(v[s * 24 + k], scale) * d;
+    }
+}
+void orc_q16_links(float *U, long nlinks)
+{
+    const float d = 1.0f / 32767.0f;
+#pragma omp parallel for schedule(static)
+    for (long l = 0; l < nlinks; l++) {
+        float *u = U + l * 18;
+        for (int k = 0; k < 12; k++) u[k] = q16_code(u[k], 32767.0f) * d;
+        /* row 2 = conj(row0 x row1), written out component by component */
+        const float complex a0 = u[0] + I * u[1], a1 = u[2] + I * u[3], a2 = u[4] + I * u[5];
+        const float complex b0 = u[6] + I * u[7], b1 = u[8] + I * u[9], b2 = u[10] + I * u[11];
+        const float complex c0 = conjf(a1 * b2 - a2 * b1), c1 = conjf(a2 * b0 - a0 * b2), c2 = conjf(a0 * b1 - a1 * b0);
+        u[12] = crealf(c0); u[13] = cimagf(c0);
+        u[14] = crealf(c1); u[15] = cimagf(c1);
+        u[16] = crealf(c2); u[17] = cimagf(c2);
+    }
+}
+void orc_q16_clover(float *A_, long nsites)
+{
+#pragma omp parallel for schedule(static)
+    for (long s = 0; s < nsites; s++) {
+        fc *A = (fc *)A_ + s * 144;
+        float n = 0.0f;
+        for (int b = 0; b < 2; b++)
+            for (int i = 0; i < 6; i++)
+                for (int j = 0; j <= i; j++) {
+                    const fc a = A[(6 * b + i) * 12 + 6 * b + j];
+                    n = fmaxf(n, fabsf(crealf(a)));
+                    if (j < i) n = fmaxf(n, fabsf(cimagf(a)));
+                }
+        const float scale = n > 0.0f ? 32767.0f / n : 0.0f, d = n / 32767.0f;
+        fc Q[144];
+        for (int k = 0; k < 144; k++) Q[k] = 0;
+        for (int b = 0; b < 2; b++)
+            for (int i = 0; i < 6; i++)
+                for (int j = 0; j <= i; j++) {
+                    const int r = 6 * b + i, c = 6 * b + j;
+                    const fc a = A[r * 12 + c];
+                    const float re = q16_code(crealf(a), scale) * d;
+                    const float im = (j < i) ? q16_code(cimagf(a), scale) * d : 0.0f;
+                    Q[r * 12 + c] = re + I * im;
+                    if (j < i) Q[c * 12 + r] = re - I * im;
+                }
+        for (int k = 0; k < 144; k++) A[k] = Q[k];
+    }
+}
+
+/* out = M in (or M^dag in) with 16-bit storage of every field the operator streams: `in` must
+ * already be a stored-and-read-back field, op holds stored-and-read-back links / clover; the
+ * intermediate of the even-odd form is stored in 16 bits, and so is the result when
+ * store_out != 0 (it is the input of the next operator).  Arithmetic fp32. */
+static void apply_M_q16(fc *out, const fc *in, const orc_op_f32 *op, int dagger, int store_out, fc *t1, fc *t2)
+{
+    const long V = (long)op->dims[0] * op->dims[1] * op->dims[2] * op->dims[3];
+    const long n = V * 12;
+    if (op->mode == 2) {
+        orc_apply_M_f32(out, in, op, dagger, t1, t2);
+    } else {
+        const int p = op->mode, pb = 1 - op->mode;
+        orc_hop_f32(t1, in, op->U, op->dims, op->tb, dagger, pb);
+        orc_site_matrix_apply_f32(t2, op->Ainv, t1, op->dims, pb);
+        orc_q16_spinor((float *)t2, V);
+        orc_hop_f32(t1, t2, op->U, op->dims, op->tb, dagger, p);
+        orc_site_matrix_apply_f32(t2, op->A, in, op->dims, p);
+        const float k2 = (float)(op->kappa * op->kappa);
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < n; i++) out[i] = t2[i] - k2 * t1[i];
+    }
+    if (store_out) orc_q16_spinor((float *)out, V);
+}
+/* q = N_16 p :  ph = store(p);  t = store(M ph);  q = M^dag t  (q left in fp32) */
+static void apply_N_q16(fc *q, const fc *p, const orc_op_f32 *op, fc *tmp, fc *t1, fc *t2, fc *ph)
+{
+    const long V = (long)op->dims[0] * op->dims[1] * op->dims[2] * op->dims[3];
+    memcpy(ph, p, (size_t)V * 12 * sizeof(fc));
+    orc_q16_spinor((float *)ph, V);
+    apply_M_q16(tmp, ph, op, 0, 1, t1, t2);
+    apply_M_q16(q, tmp, op, 1, 0, t1, t2);
+}
+int orc_apply_N_q16(float *q, const float *p, const float *U, const float *A, const float *Ainv, const int *dims,
+                    double kappa, int tb, int mode)
+{
+    const long n = (long)dims[0] * dims[1] * dims[2] * dims[3] * 12;
+    orc_op_f32 op;
+    fill_op32(&op, U, A, Ainv, dims, kappa, tb, mode);
+    fc *tmp = malloc(n * sizeof(fc)), *t1 = malloc(n * sizeof(fc)), *t2 = malloc(n * sizeof(fc)), *ph = malloc(n * sizeof(fc));
+    if (!tmp || !t1 || !t2 || !ph) { free(tmp); free(t1); free(t2); free(ph); return -1; }
+    orc_init_gamma();
+    apply_N_q16((fc *)q, (const fc *)p, &op, tmp, t1, t2, ph);
+    free(tmp); free(t1); free(t2); free(ph);
+    return 0;
+}
+int orc_apply_M_q16(float *out, const float *in, const float *U, const float *A, const float *Ainv, const int *dims,
+                    double kappa, int tb, int mode, int dagger, int store_out)
+{
+    const long n = (long)dims[0] * dims[1] * dims[2] * dims[3] * 12;
+    orc_op_f32 op;
+    fill_op32(&op, U, A, Ainv, dims, kappa, tb, mode);
+    fc *t1 = malloc(n * sizeof(fc)), *t2 = malloc(n * sizeof(fc));
+    if (!t1 || !t2) { free(t1); free(t2); return -1; }
+    orc_init_gamma();
+    apply_M_q16((fc *)out, (const fc *)in, &op, dagger, store_out, t1, t2);
+    free(t1); free(t2);
     return 0;
 }
 
