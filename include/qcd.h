@@ -18,7 +18,8 @@
  *  - Every field pointer is a DEVICE pointer owned by the caller, 16-byte aligned.
  *    The library never allocates field-sized memory; handles are small host structs.
  *    (qcd_*_host entry points take HOST pointers and say so.)
- *  - dims = {X,Y,Z,T}, all even and >= 2.  precision = bytes per real: 4 or 8.
+ *  - dims = {X,Y,Z,T}, all even and >= 2.  precision = bytes per real: 4 or 8 (2 = the
+ *    16-bit storage of the low-precision operator, where a function says so).
  *  - Boundary (user) layouts, real type = precision:
  *      gauge  [t][z][y][x][mu=0..3 (x,y,z,t)][row][col][re,im]
  *      spinor [t][z][y][x][spin 0..3][colour 0..2][re,im]
@@ -143,6 +144,24 @@ int qcd_dslash(void* out, const void* in, const qcd_gauge* gauge, const qcd_clov
                double kappa, double csw, int parity, const int dims[4], int precision);
 int qcd_dslash_ex(void* out, const void* in, const qcd_gauge* gauge, const qcd_clover* clover,
                   double kappa, double csw, int parity, int flags, void* tmp);
+
+/* ---- 16-bit storage of the low-precision operator (PAPER.md:163 ref. [1]) --------
+ * precision = 2 in qcd_gauge_load (12-real only) and qcd_clover_build selects 16-bit
+ * fixed-point storage (reading H1 in DESIGN.md): int16 codes, a per-site fp32 norm for
+ * spinors and clover blocks, scale 32767 for links; arithmetic stays fp32.
+ * A 16-bit spinor field is nblocks parity blocks of [3 x int4][Vh] codes + [Vh] fp32 norms
+ * (52 bytes per site).  qcd_spinor_to_half / _from_half convert an fp32 internal field.
+ * qcd_dslash_half: out = M in (or M^dag) as qcd_dslash_ex, with the 16-bit gauge / clover
+ * handles, `in_half` a 16-bit field, the even-odd intermediate stored in 16 bits in
+ * `tmp_half` (one parity block; parity 0|1 only) and `out` a 16-bit (out_precision = 2) or
+ * fp32 (4) field.  Passing 16-bit handles as g_lo / c_lo to qcd_set_operator makes
+ * qcd_cg_solve run the reliable-update CG with this operator inside (inner vectors fp32). */
+size_t qcd_half_spinor_bytes(const int dims[4]);   /* full lattice */
+int qcd_spinor_to_half(qcd_ctx* ctx, void* half, const void* f32, const int dims[4], int nblocks);
+int qcd_spinor_from_half(qcd_ctx* ctx, void* f32, const void* half, const int dims[4], int nblocks);
+int qcd_dslash_half(void* out, int out_precision, const void* in_half, const qcd_gauge* gauge,
+                    const qcd_clover* clover, double kappa, double csw, int parity, int flags,
+                    void* tmp_half);
 
 /* ---- workspace ----------------------------------------------------------------------
  * Caller-provided DEVICE scratch used by qcd_dslash (parity 0|1), the solvers and the

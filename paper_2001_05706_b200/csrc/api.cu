@@ -98,6 +98,7 @@ size_t qcd_gauge_bytes(const int dims[4], int precision, int reconstruct)
 {
     Geom g;
     if (make_geom(dims, &g) != QCD_OK) return 0;
+    if (precision == 2) return reconstruct == 12 ? 8 * gauge_block_bytes(g, 2, 12) : 0;
     if ((precision != 4 && precision != 8) || (reconstruct != 12 && reconstruct != 18)) return 0;
     return 8 * gauge_block_bytes(g, precision, reconstruct);
 }
@@ -110,9 +111,10 @@ int qcd_gauge_load(qcd_ctx* ctx, qcd_gauge** out, const void* links, int precisi
     Geom g;
     int rc = make_geom(dims, &g);
     if (rc) return rc;
-    QCD_REQUIRE(precision == 4 || precision == 8, "gauge_load: precision must be 4|8");
+    QCD_REQUIRE(precision == 2 || precision == 4 || precision == 8, "gauge_load: precision must be 2|4|8");
     QCD_REQUIRE(precision_in == 4 || precision_in == 8, "gauge_load: precision_in must be 4|8");
     QCD_REQUIRE(reconstruct == 12 || reconstruct == 18, "gauge_load: reconstruct must be 12|18");
+    QCD_REQUIRE(precision != 2 || reconstruct == 12, "gauge_load: 16-bit links are stored with 12 reals");
     QCD_REQUIRE(t_boundary == 1 || t_boundary == -1, "gauge_load: t_boundary must be +1|-1");
     QCD_REQUIRE(aligned16(links) && aligned16(storage), "gauge_load: pointers must be non-NULL and 16-byte aligned");
     qcd_gauge* h = (qcd_gauge*)calloc(1, sizeof(qcd_gauge));
@@ -132,6 +134,7 @@ size_t qcd_clover_bytes(const int dims[4], int precision)
 {
     Geom g;
     if (make_geom(dims, &g) != QCD_OK) return 0;
+    if (precision == 2) return (size_t)4 * g.Vh * 148; /* 72 int16 codes + one fp32 norm per site */
     if (precision != 4 && precision != 8) return 0;
     return (size_t)4 * g.Vh * 72 * precision; /* A[2 parities] + Ainv[2 parities] */
 }
@@ -140,13 +143,14 @@ int qcd_clover_build(qcd_ctx* ctx, qcd_clover** out, const qcd_gauge* g, void* s
 {
     QCD_REQUIRE(ctx && out && g, "clover_build: NULL argument");
     *out = nullptr;
-    QCD_REQUIRE(precision == 4 || precision == 8, "clover_build: precision must be 4|8");
+    QCD_REQUIRE(precision == 2 || precision == 4 || precision == 8, "clover_build: precision must be 2|4|8");
+    QCD_REQUIRE(g->precision != 2, "clover_build: build from an fp32 or fp64 gauge handle");
     QCD_REQUIRE(aligned16(storage), "clover_build: storage must be non-NULL and 16-byte aligned");
     qcd_clover* c = (qcd_clover*)calloc(1, sizeof(qcd_clover));
     if (!c) return qcd_set_error(QCD_EALLOC, "clover handle");
     c->ctx = ctx; c->geo = g->geo; c->precision = precision; c->kappa = kappa; c->csw = csw;
     c->data = storage;
-    c->block_bytes = (size_t)g->geo.Vh * 72 * precision;
+    c->block_bytes = precision == 2 ? (size_t)g->geo.Vh * 148 : (size_t)g->geo.Vh * 72 * precision;
     int rc = clover_build(ctx, g, c);
     if (rc) { free(c); return rc; }
     *out = c;
@@ -223,6 +227,7 @@ int qcd_set_workspace(qcd_ctx* ctx, void* ws, size_t bytes)
 int qcd_hop_xpay(void* out, const void* in, const void* z, double a, double b, const qcd_gauge* g, int out_parity, int dagger)
 {
     QCD_REQUIRE(g && g->ctx, "hop: NULL gauge");
+    QCD_REQUIRE(g->precision != 2, "hop: 16-bit gauge handle: use qcd_dslash_half");
     const size_t bytes = (size_t)g->geo.Vh * 24 * g->precision;
     QCD_REQUIRE(aligned16(out) && aligned16(in), "hop: pointers must be non-NULL, 16-byte aligned");
     QCD_REQUIRE(!overlap(out, in, bytes), "hop: in and out alias");
@@ -300,6 +305,7 @@ int qcd_dslash_ex(void* out, const void* in, const qcd_gauge* g, const qcd_clove
                   void* tmp)
 {
     QCD_REQUIRE(g && g->ctx, "dslash: NULL gauge");
+    QCD_REQUIRE(g->precision != 2, "dslash: 16-bit gauge handle: use qcd_dslash_half");
     qcd_ctx* ctx = g->ctx;
     QCD_REQUIRE(parity == 0 || parity == 1 || parity == 2, "dslash: parity must be 0|1|2");
     QCD_REQUIRE(aligned16(out) && aligned16(in), "dslash: pointers must be non-NULL, 16-byte aligned");
@@ -326,6 +332,87 @@ int qcd_dslash(void* out, const void* in, const qcd_gauge* g, const qcd_clover* 
     QCD_REQUIRE(g, "dslash: NULL gauge");
     QCD_REQUIRE(same_dims(g->geo, dims) && precision == g->precision, "dslash: dims/precision do not match the gauge handle");
     return qcd_dslash_ex(out, in, g, c, kappa, csw, parity, 0, nullptr);
+}
+
+/* ---- 16-bit storage (reading H1) ---------------------------------------------- */
+} /* extern "C" */
+
+/* out = M in with every streamed field in 16 bits; in: 16-bit field; out: 16-bit or fp32 */
+int op_apply_M_half(qcd_ctx* ctx, void* out, int out_f32, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c,
+                    double kappa, int parity, int dagger)
+{
+    const size_t hblk = (size_t)g->geo.Vh * 52, oblk = out_f32 ? (size_t)g->geo.Vh * 96 : hblk;
+    HopLaunch L;
+    if (parity == QCD_PARITY_FULL) {
+        for (int p = 0; p < 2; p++) {
+            memset(&L, 0, sizeof(L));
+            L.out = (char*)out + p * oblk;
+            L.in = (const char*)in + (1 - p) * hblk;
+            L.z = (const char*)in + p * hblk;
+            L.a = 1.0; L.b = -kappa; L.out_parity = p; L.dagger = dagger;
+            if (c) { L.mode = HOP_CLOVER_Z; L.clover = (const char*)c->data + p * c->block_bytes; }
+            else L.mode = HOP_XPAY;
+            int rc = hop_half_launch(ctx, g, L, out_f32);
+            if (rc) return rc;
+        }
+        return QCD_OK;
+    }
+    const int p = parity;
+    memset(&L, 0, sizeof(L));
+    L.out = tmp; L.in = in; L.out_parity = 1 - p; L.dagger = dagger;
+    if (c) { L.mode = HOP_CLOVER_OUT; L.clover = (const char*)c->data + (2 + (1 - p)) * c->block_bytes; }
+    else L.mode = HOP_PLAIN;
+    int rc = hop_half_launch(ctx, g, L, 0);
+    if (rc) return rc;
+    memset(&L, 0, sizeof(L));
+    L.out = out; L.in = tmp; L.z = in; L.a = 1.0; L.b = -kappa * kappa; L.out_parity = p; L.dagger = dagger;
+    if (c) { L.mode = HOP_CLOVER_Z; L.clover = (const char*)c->data + p * c->block_bytes; }
+    else L.mode = HOP_XPAY;
+    return hop_half_launch(ctx, g, L, out_f32);
+}
+
+extern "C" {
+
+size_t qcd_half_spinor_bytes(const int dims[4])
+{
+    Geom g;
+    if (make_geom(dims, &g) != QCD_OK) return 0;
+    return (size_t)g.V * 52;
+}
+
+int qcd_spinor_to_half(qcd_ctx* ctx, void* half, const void* f32, const int dims[4], int nblocks)
+{
+    QCD_REQUIRE(ctx && aligned16(half) && aligned16(f32), "spinor_to_half: bad pointer");
+    QCD_REQUIRE(nblocks == 1 || nblocks == 2, "spinor_to_half: nblocks must be 1|2");
+    Geom g;
+    int rc = make_geom(dims, &g);
+    if (rc) return rc;
+    return half_convert(ctx, half, const_cast<void*>(f32), (size_t)g.Vh, nblocks, 1);
+}
+
+int qcd_spinor_from_half(qcd_ctx* ctx, void* f32, const void* half, const int dims[4], int nblocks)
+{
+    QCD_REQUIRE(ctx && aligned16(half) && aligned16(f32), "spinor_from_half: bad pointer");
+    QCD_REQUIRE(nblocks == 1 || nblocks == 2, "spinor_from_half: nblocks must be 1|2");
+    Geom g;
+    int rc = make_geom(dims, &g);
+    if (rc) return rc;
+    return half_convert(ctx, const_cast<void*>(half), f32, (size_t)g.Vh, nblocks, 0);
+}
+
+int qcd_dslash_half(void* out, int out_precision, const void* in_half, const qcd_gauge* g, const qcd_clover* c, double kappa, double csw,
+                    int parity, int flags, void* tmp_half)
+{
+    QCD_REQUIRE(g && g->ctx && g->precision == 2, "dslash_half: needs a 16-bit gauge handle");
+    QCD_REQUIRE(out_precision == 2 || out_precision == 4, "dslash_half: out_precision must be 2|4");
+    QCD_REQUIRE(parity == 0 || parity == 1 || parity == 2, "dslash_half: parity must be 0|1|2");
+    QCD_REQUIRE(aligned16(out) && aligned16(in_half) && out != in_half, "dslash_half: bad in/out pointer");
+    if (c) {
+        QCD_REQUIRE(c->precision == 2 && c->geo.V == g->geo.V, "dslash_half: needs a 16-bit clover handle of the same lattice");
+        QCD_REQUIRE(c->kappa == kappa && c->csw == csw, "dslash_half: kappa/csw differ from the values the clover was built with");
+    }
+    if (parity != 2) QCD_REQUIRE(aligned16(tmp_half) && tmp_half != out && tmp_half != in_half, "dslash_half: parity 0|1 needs tmp_half");
+    return op_apply_M_half(g->ctx, out, out_precision == 4, in_half, tmp_half, g, c, kappa, parity, (flags & QCD_DAGGER) ? 1 : 0);
 }
 
 /* ---- BLAS ------------------------------------------------------------------------------ */

@@ -12,8 +12,9 @@
  * All arithmetic here is fp64 whatever the storage precision.
  */
 #include <math.h>
+#include <type_traits>
 
-#include "qcd_device.cuh"
+#include "half_device.cuh"
 
 namespace {
 
@@ -165,6 +166,34 @@ template <typename TS> __device__ void store_block(TS* blk, size_t Vh, size_t cb
     store_planes<TS, 36>(blk + (size_t)36 * b * Vh, Vh, cb, r);
 }
 
+/* tag type: 16-bit storage (reading H1) */
+struct HalfTag {};
+
+/* pack both chiral blocks of a site (72 reals, fp32) */
+__device__ void pack_site(float (&r)[72], cplx (*a)[6][6])
+{
+    for (int b = 0; b < 2; b++) {
+        for (int i = 0; i < 6; i++) r[36 * b + i] = (float)a[b][i][i].re;
+        for (int lo = 0; lo < 6; lo++)
+            for (int hi = lo + 1; hi < 6; hi++) {
+                const int k = 36 * b + 6 + 2 * tri_index(hi, lo);
+                r[k] = (float)(0.5 * (a[b][hi][lo].re + a[b][lo][hi].re));
+                r[k + 1] = (float)(0.5 * (a[b][hi][lo].im - a[b][lo][hi].im));
+            }
+    }
+}
+__device__ void store_site_half(unsigned char* blk, size_t Vh, size_t cb, cplx (*a)[6][6])
+{
+    float r[72];
+    pack_site(r, a);
+    float n = 0.f;
+    for (int k = 0; k < 72; k++) n = fmaxf(n, fabsf(r[k]));
+    const float scale = n > 0.f ? __fdiv_rn(32767.0f, n) : 0.f;
+    int4* q = reinterpret_cast<int4*>(blk) + cb;
+    for (int c = 0; c < 9; c++) q[(size_t)c * Vh] = half_pack8(&r[8 * c], scale);
+    reinterpret_cast<float*>(blk + Vh * 144)[cb] = n;
+}
+
 template <typename T, int RECON, typename TS>
 __global__ void __launch_bounds__(64) clover_build_kernel(LinkReader<T, RECON> R, TS* A, TS* Ainv, size_t cblock, double coeff, int* bad)
 {
@@ -213,17 +242,21 @@ __global__ void __launch_bounds__(64) clover_build_kernel(LinkReader<T, RECON> R
                     }
         }
 
-    for (int b = 0; b < 2; b++) {
+    for (int b = 0; b < 2; b++)
         for (int r = 0; r < 6; r++)
             for (int s = 0; s < 6; s++) {
                 blk[b][r][s].re *= coeff;
                 blk[b][r][s].im *= coeff;
                 if (r == s) blk[b][r][s].re += 1.0;
             }
-        store_block<TS>(A + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, b, blk[b]);
+    constexpr bool HALF = std::is_same<TS, HalfTag>::value;
+    if constexpr (HALF) store_site_half(reinterpret_cast<unsigned char*>(A) + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, blk);
+    for (int b = 0; b < 2; b++) {
+        if constexpr (!HALF) store_block<TS>(A + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, b, blk[b]);
         if (!invert6(blk[b])) atomicAdd(bad, 1);
-        store_block<TS>(Ainv + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, b, blk[b]);
+        if constexpr (!HALF) store_block<TS>(Ainv + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, b, blk[b]);
     }
+    if constexpr (HALF) store_site_half(reinterpret_cast<unsigned char*>(Ainv) + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, blk);
 }
 
 /* expand packed blocks to dense 12x12 complex per site, boundary site order, fp64 */
@@ -254,6 +287,33 @@ template <typename TS> __global__ void clover_unpack_kernel(double* dense, const
     }
 }
 
+__global__ void clover_unpack_half_kernel(double* dense, const unsigned char* C, size_t cblock, DevGeom g)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * g.Vh) return;
+    const int parity = i / g.Vh, cb = i - parity * g.Vh;
+    const Coord c = cb_to_coord(g, cb, parity);
+    const size_t s = (size_t)c.x + (size_t)g.X * (c.y + (size_t)g.Y * (c.z + (size_t)g.Z * c.t));
+    double* d = dense + s * 288;
+    for (int k = 0; k < 288; k++) d[k] = 0.0;
+    for (int b = 0; b < 2; b++) {
+        float r[36];
+        half_load_clover_block(r, C + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, b);
+        for (int ii = 0; ii < 6; ii++) {
+            const int row = 6 * b + ii;
+            d[(row * 12 + row) * 2] = (double)r[ii];
+            for (int jj = 0; jj < ii; jj++) {
+                const int col = 6 * b + jj;
+                const int k = 6 + 2 * tri_index(ii, jj);
+                d[(row * 12 + col) * 2] = (double)r[k];
+                d[(row * 12 + col) * 2 + 1] = (double)r[k + 1];
+                d[(col * 12 + row) * 2] = (double)r[k];
+                d[(col * 12 + row) * 2 + 1] = -(double)r[k + 1];
+            }
+        }
+    }
+}
+
 template <typename T, int RECON>
 cudaError_t build_launch(qcd_ctx* ctx, const qcd_gauge* gh, const qcd_clover* c, int* d_bad)
 {
@@ -263,7 +323,12 @@ cudaError_t build_launch(qcd_ctx* ctx, const qcd_gauge* gh, const qcd_clover* c,
     R.g = dev_geom(gh->geo);
     const int threads = 64, blocks = (2 * R.g.Vh + threads - 1) / threads;
     const double coeff = c->kappa * c->csw;
-    if (c->precision == 4) {
+    if (c->precision == 2) {
+        /* cblock in bytes; A, Ainv addressed as bytes inside the kernel */
+        HalfTag* A = (HalfTag*)c->data;
+        clover_build_kernel<T, RECON, HalfTag><<<blocks, threads, 0, ctx->stream>>>(R, A, (HalfTag*)((unsigned char*)c->data + 2 * c->block_bytes),
+                                                                                 c->block_bytes, coeff, d_bad);
+    } else if (c->precision == 4) {
         const size_t cblock = c->block_bytes / 4;
         float* A = (float*)c->data;
         clover_build_kernel<T, RECON, float><<<blocks, threads, 0, ctx->stream>>>(R, A, A + 2 * cblock, cblock, coeff, d_bad);
@@ -300,7 +365,10 @@ int clover_unpack(qcd_ctx* ctx, void* dense, const qcd_clover* c, int which)
 {
     const DevGeom g = dev_geom(c->geo);
     const int threads = 64, blocks = (2 * g.Vh + threads - 1) / threads;
-    if (c->precision == 4) {
+    if (c->precision == 2) {
+        clover_unpack_half_kernel<<<blocks, threads, 0, ctx->stream>>>((double*)dense, (const unsigned char*)c->data + (which ? 2 * c->block_bytes : 0),
+                                                                     c->block_bytes, g);
+    } else if (c->precision == 4) {
         const size_t cblock = c->block_bytes / 4;
         clover_unpack_kernel<float><<<blocks, threads, 0, ctx->stream>>>((double*)dense, (const float*)c->data + (which ? 2 * cblock : 0), cblock, g);
     } else {

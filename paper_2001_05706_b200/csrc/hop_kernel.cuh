@@ -36,6 +36,13 @@ template <typename T> struct HopArgs {
     T a, b, c1, c2, c3;
 };
 
+/* ---- where a neighbour spinor comes from ---------------------------------------------- */
+template <typename T> struct PlaneSpinor {
+    const T* base;
+    size_t Vh;
+    __device__ __forceinline__ void load(T (&s)[24], int idx) const { load_planes<T, 24>(s, base, Vh, (size_t)idx); }
+};
+
 /* ---- where a direction's link comes from ------------------------------------------- */
 template <typename T, int RECON> struct GlobalLinks {
     const T* gauge;
@@ -169,11 +176,11 @@ __device__ __forceinline__ void colour_mul(T (&w)[12], const T (&u)[18], const T
 }
 
 /* one direction: MU, DIR = +1 forward / -1 backward; SG = projector sign (forward: -1, i.e. 1 - g) */
-template <typename T, int MU, int DIR, int SG, typename Links>
-__device__ __forceinline__ void hop_dir(T (&acc)[24], const Links& L, const T* __restrict__ in, size_t Vh, int cb, int nb_cb, T sign)
+template <typename T, int MU, int DIR, int SG, typename Links, typename Src>
+__device__ __forceinline__ void hop_dir(T (&acc)[24], const Links& L, const Src& in, int cb, int nb_cb, T sign)
 {
     T s[24], u[18], h[12], w[12];
-    load_planes<T, 24>(s, in, Vh, (size_t)nb_cb);
+    in.load(s, nb_cb);
     L.template get<MU, DIR>(u, cb, nb_cb);
     project<T, MU, SG>(h, s);
     colour_mul<T, (DIR < 0)>(w, u, h, sign);
@@ -235,22 +242,22 @@ template <typename T> struct Neighbours {
 };
 
 /* acc = (H in)(cb) (or H^dag): the eight directions */
-template <typename T, int DAG, typename Links>
-__device__ __forceinline__ void hop_site(T (&acc)[24], const Links& L, const T* __restrict__ in, size_t Vh, int cb, const Neighbours<T>& n)
+template <typename T, int DAG, typename Links, typename Src>
+__device__ __forceinline__ void hop_site(T (&acc)[24], const Links& L, const Src& in, int cb, const Neighbours<T>& n)
 {
     /* forward hop carries (1 - g_mu), backward (1 + g_mu); the adjoint swaps them (O4) */
     constexpr int SF = DAG ? +1 : -1;
     constexpr int SB = DAG ? -1 : +1;
 #pragma unroll
     for (int i = 0; i < 24; i++) acc[i] = 0;
-    hop_dir<T, 0, +1, SF>(acc, L, in, Vh, cb, n.xp, (T)1);
-    hop_dir<T, 0, -1, SB>(acc, L, in, Vh, cb, n.xm, (T)1);
-    hop_dir<T, 1, +1, SF>(acc, L, in, Vh, cb, n.yp, (T)1);
-    hop_dir<T, 1, -1, SB>(acc, L, in, Vh, cb, n.ym, (T)1);
-    hop_dir<T, 2, +1, SF>(acc, L, in, Vh, cb, n.zp, (T)1);
-    hop_dir<T, 2, -1, SB>(acc, L, in, Vh, cb, n.zm, (T)1);
-    hop_dir<T, 3, +1, SF>(acc, L, in, Vh, cb, n.tp, n.sgn_tp);
-    hop_dir<T, 3, -1, SB>(acc, L, in, Vh, cb, n.tm, n.sgn_tm);
+    hop_dir<T, 0, +1, SF>(acc, L, in, cb, n.xp, (T)1);
+    hop_dir<T, 0, -1, SB>(acc, L, in, cb, n.xm, (T)1);
+    hop_dir<T, 1, +1, SF>(acc, L, in, cb, n.yp, (T)1);
+    hop_dir<T, 1, -1, SB>(acc, L, in, cb, n.ym, (T)1);
+    hop_dir<T, 2, +1, SF>(acc, L, in, cb, n.zp, (T)1);
+    hop_dir<T, 2, -1, SB>(acc, L, in, cb, n.zm, (T)1);
+    hop_dir<T, 3, +1, SF>(acc, L, in, cb, n.tp, n.sgn_tp);
+    hop_dir<T, 3, -1, SB>(acc, L, in, cb, n.tm, n.sgn_tm);
 }
 
 #ifndef HOP_MINBLOCKS_F32
@@ -268,8 +275,9 @@ __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? HOP_MINBLOCKS_F32 : HOP
     const size_t Vh = (size_t)A.geo.Vh;
     const Neighbours<T> nb(A.geo, cb, A.parity, A.tb);
     const GlobalLinks<T, RECON> L = {A.gauge, A.gblock, Vh, A.parity};
+    const PlaneSpinor<T> src = {A.in, Vh};
     T acc[24];
-    hop_site<T, DAG>(acc, L, A.in, Vh, cb, nb);
+    hop_site<T, DAG>(acc, L, src, cb, nb);
 
     if (MODE == HOP_PLAIN) {
         store_planes<T, 24>(A.out, Vh, (size_t)cb, acc);
@@ -302,8 +310,9 @@ __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? HOP_MINBLOCKS_F32 : HOP
 template <typename T, typename Links>
 __device__ __forceinline__ void cheb_vector(const HopArgs<T>& A, const Links& L, size_t off, size_t Vh, int cb, const Neighbours<T>& nb)
 {
+    const PlaneSpinor<T> src = {A.in + off, Vh};
     T acc[24], zz[24];
-    hop_site<T, 0>(acc, L, A.in + off, Vh, cb, nb);
+    hop_site<T, 0>(acc, L, src, cb, nb);
     load_planes_cs<T, 24>(zz, A.z + off, Vh, (size_t)cb);
 #pragma unroll
     for (int i = 0; i < 24; i++) {

@@ -112,6 +112,14 @@ int hop_launch(qcd_ctx* ctx, const qcd_gauge* g, const HopLaunch& L);
 int op_apply_M(qcd_ctx* ctx, void* out, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c,
                double kappa, int parity, int dagger);
 
+/* ---- 16-bit storage path (hop_half.cu, api.cu) ---------------------------- */
+int hop_half_launch(qcd_ctx* ctx, const qcd_gauge* g, const HopLaunch& L, int out_f32);
+int half_convert(qcd_ctx* ctx, void* half, void* f32, size_t Vh, int nblocks, int to_half);
+/* p = a r + b p (fp32) ; ph = 16-bit copy of p */
+int half_xpay_store(qcd_ctx* ctx, double a, const void* r, double b, void* p, void* ph, size_t Vh, int nblocks);
+int op_apply_M_half(qcd_ctx* ctx, void* out, int out_f32, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c,
+                    double kappa, int parity, int dagger);
+
 /* ---- blas.cu --------------------------------------------------------------------- */
 /* A scalar that is either a host value or the quotient of two device doubles. */
 struct DevScalar {
@@ -165,7 +173,7 @@ int clover_unpack(qcd_ctx*, void* dense, const qcd_clover* c, int which);
 
 static inline size_t gauge_block_bytes(const Geom& g, int precision, int reconstruct)
 {
-    return (size_t)g.Vh * (size_t)reconstruct * (size_t)precision;
+    return (size_t)g.Vh * (size_t)reconstruct * (size_t)precision; /* precision 2: 12 int16 codes = 24 B */
 }
 
 #endif

@@ -127,14 +127,22 @@ int cg_pure(qcd_ctx* ctx, void* x, const void* b, double tol, int maxiter, qcd_s
 int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_stats* st)
 {
     const Op oh = make_op(ctx, ctx->g_hi, ctx->c_hi);
-    const Op ol = make_op(ctx, ctx->g_lo, ctx->c_lo);
-    QCD_REQUIRE(oh.g->precision == 8 && ol.g->precision == 4, "mixed cg: needs an fp64 high and an fp32 low operator");
+    Op ol = make_op(ctx, ctx->g_lo, ctx->c_lo);
+    QCD_REQUIRE(oh.g->precision == 8 && (ol.g->precision == 4 || ol.g->precision == 2),
+                "mixed cg: needs an fp64 high and an fp32 or 16-bit low operator");
+    /* 16-bit low operator (reading H1): the inner vectors stay fp32, the operator streams 16-bit fields */
+    const bool half = ol.g->precision == 2;
+    ol.bytes = ol.nreal * 4;
+    const int nblocks = ol.parity == 2 ? 2 : 1;
     const size_t need = 4 * oh.bytes + 6 * ol.bytes;
     QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= need, "mixed cg: workspace too small (need %zu bytes)", need);
     char* w = (char*)ctx->ws;
     void *rh = w, *th = w + oh.bytes, *h1 = w + 2 * oh.bytes, *h2 = w + 3 * oh.bytes;
     char* wl = w + 4 * oh.bytes;
     void *x = wl, *r = wl + ol.bytes, *p = wl + 2 * ol.bytes, *q = wl + 3 * ol.bytes, *tl = wl + 4 * ol.bytes, *l2 = wl + 5 * ol.bytes;
+    /* 16-bit operator buffers share the tl/l2 region: 3 x 52 B/site < 2 x 96 B/site */
+    const size_t hbytes = (size_t)nblocks * ol.g->geo.Vh * 52;
+    char *ph = (char*)tl, *th16 = ph + hbytes, *tmp16 = th16 + hbytes;
     double* d = ctx->d_scalar;
     double* h = ctx->h_scalar;
     const size_t n = oh.nreal, Vh = (size_t)oh.g->geo.Vh;
@@ -143,7 +151,8 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
     RC(blas_zero(ctx, y, oh.bytes));
     RC(blas_zero(ctx, x, ol.bytes));
     RC(blas_convert(ctx, r, 4, b, 8, n, Vh));
-    RC(blas_copy(ctx, p, r, ol.bytes));
+    if (half) RC(half_xpay_store(ctx, 1.0, r, 0.0, p, ph, Vh, nblocks));
+    else RC(blas_copy(ctx, p, r, ol.bytes));
     int cur = S_RHO_A, nxt = S_RHO_B;
     RC(blas_norm2(ctx, b, n, 8, d + S_AUX));
     RC(blas_norm2(ctx, r, n, 4, d + cur));
@@ -155,7 +164,12 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
     const bool trace = getenv("QCD_TRACE") != nullptr;
     while (!conv && k < maxiter) {
         k++;
-        RC(apply_N(ol, q, p, tl, l2));
+        if (half) {
+            RC(op_apply_M_half(ctx, th16, 0, ph, tmp16, ol.g, ol.c, ol.kappa, ol.parity, 0));
+            RC(op_apply_M_half(ctx, q, 1, th16, tmp16, ol.g, ol.c, ol.kappa, ol.parity, 1));
+        } else {
+            RC(apply_N(ol, q, p, tl, l2));
+        }
         RC(blas_redot(ctx, p, q, n, 4, d + S_PQ));
         RC(blas_cg_update(ctx, dev_ratio(d + cur, d + S_PQ), p, q, x, r, n, 4, d + nxt, nullptr, nullptr));
         RC(fetch(ctx, 0, 4));
@@ -177,7 +191,8 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
             if (rhnorm <= tol * bnorm) { conv = 1; break; }
         }
         const float beta = (float)(rho2 / rho);
-        RC(blas_axpby(ctx, host_scalar(1.0), r, host_scalar((double)beta), p, n, 4));
+        if (half) RC(half_xpay_store(ctx, 1.0, r, (double)beta, p, ph, Vh, nblocks));
+        else RC(blas_axpby(ctx, host_scalar(1.0), r, host_scalar((double)beta), p, n, 4));
         rho = rho2;
         const int s = cur; cur = nxt; nxt = s;
     }

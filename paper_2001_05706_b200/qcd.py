@@ -59,6 +59,10 @@ SIGNATURES = {
     "qcd_hop_xpay": (_i, [_vp, _vp, _vp, _d, _d, _vp, _i, _i]),
     "qcd_dslash": (_i, [_vp, _vp, _vp, _vp, _d, _d, _i, _dims_t, _i]),
     "qcd_dslash_ex": (_i, [_vp, _vp, _vp, _vp, _d, _d, _i, _i, _vp]),
+    "qcd_half_spinor_bytes": (_sz, [_dims_t]),
+    "qcd_spinor_to_half": (_i, [_vp, _vp, _vp, _dims_t, _i]),
+    "qcd_spinor_from_half": (_i, [_vp, _vp, _vp, _dims_t, _i]),
+    "qcd_dslash_half": (_i, [_vp, _i, _vp, _vp, _vp, _d, _d, _i, _i, _vp]),
     "qcd_workspace_bytes": (_sz, [_dims_t, _i]),
     "qcd_set_workspace": (_i, [_vp, _vp, _sz]),
     "qcd_axpy": (_i, [_vp, _d, _vp, _vp, _sz, _i]),
@@ -217,6 +221,23 @@ class Context:
     def dslash_ex(self, out, inp, gauge: "Gauge", clover, kappa: float, csw: float, parity: int, flags: int = 0, tmp=None):
         _check(lib().qcd_dslash_ex(_ptr(out), _ptr(inp), gauge.h, clover.h if clover else None, kappa, csw, parity,
                                    flags, _ptr(tmp)))
+
+    # ---- 16-bit storage ---------------------------------------------------------------
+    def spinor_to_half(self, f32: torch.Tensor, dims, nblocks: int) -> torch.Tensor:
+        half = self.empty(lib().qcd_half_spinor_bytes(_dims(dims)) // 2 * nblocks)
+        _check(lib().qcd_spinor_to_half(self.h, _ptr(half), _ptr(f32), _dims(dims), nblocks))
+        return half
+
+    def spinor_from_half(self, half: torch.Tensor, dims, nblocks: int) -> torch.Tensor:
+        X, Y, Z, T = (int(d) for d in dims)
+        f32 = torch.empty(nblocks * (X * Y * Z * T // 2) * 24, dtype=torch.float32, device=self.device)
+        _check(lib().qcd_spinor_from_half(self.h, _ptr(f32), _ptr(half), _dims(dims), nblocks))
+        return f32
+
+    def dslash_half(self, out, out_precision: int, in_half, gauge: "Gauge", clover, kappa: float, csw: float, parity: int,
+                    flags: int = 0, tmp_half=None):
+        _check(lib().qcd_dslash_half(_ptr(out), out_precision, _ptr(in_half), gauge.h, clover.h if clover else None,
+                                     kappa, csw, parity, flags, _ptr(tmp_half)))
 
     def hop_host(self, out_host, in_host, gauge: "Gauge", out_parity: int, dagger: bool = False):
         """out_host / in_host: pinned (or pageable) HOST tensors, one-parity internal blocks."""

@@ -46,7 +46,12 @@ def test_size_queries(qcd):
     # odd or too small extents, bad precision
     assert L.qcd_gauge_bytes(qcd._dims((3, 4, 4, 4)), 4, 12) == 0
     assert L.qcd_gauge_bytes(qcd._dims((4, 4, 4, 0)), 4, 12) == 0
-    assert L.qcd_gauge_bytes(d, 2, 12) == 0
+    assert L.qcd_gauge_bytes(d, 3, 12) == 0
+    # 16-bit storage (reading H1): 24 B per link, 148 B per clover site and block, 52 B per spinor site
+    assert L.qcd_gauge_bytes(d, 2, 12) == 8 * (V // 2) * 24
+    assert L.qcd_gauge_bytes(d, 2, 18) == 0
+    assert L.qcd_clover_bytes(d, 2) == 4 * (V // 2) * 148
+    assert L.qcd_half_spinor_bytes(d) == V * 52
     assert L.qcd_gauge_bytes(d, 4, 8) == 0
 
 
