@@ -221,6 +221,8 @@ def build_workload(c, dims, want_hi):
         w["g32_18"] = c.gauge_load(dU, dims, 4, 18, -1)
         w["g64"] = g_hi
         w["c64"] = c.clover_build(g_hi, KAPPA, CSW, 8)
+        w["g16"] = c.gauge_load(dU, dims, 2, 12, -1)           # 16-bit storage (reading H1)
+        w["c16"] = c.clover_build(g_hi, KAPPA, CSW, 2)
     del dU
     psi = torch.from_numpy(inputs.spinor_field(dims, 0, 0))
     w["psi64"] = c.spinor_pack(psi.cuda(), dims) if want_hi else None
@@ -267,6 +269,14 @@ def kernel_table(c, w, peak):
     tmp64 = torch.empty_like(b64)
     ms = gpu_time_ms(lambda: c.dslash_ex(b64, a64, w["g64"], w["c64"], KAPPA, CSW, 0, 0, tmp64), 20)
     row("Mhat_clover_fp64_18 (2 launches)", ms, 2 * 1536 + 2 * 576 + 192, 2 * 1320 + 2 * 504)
+    # 16-bit storage (reading H1): 52 B spinor site, 24 B link, 148 B clover site
+    ph = c.spinor_to_half(w["psi32"], dims, 2)
+    hb = Vh * 52
+    o16, t16 = c.empty(hb), c.empty(hb)
+    ms = gpu_time_ms(lambda: c.dslash_half(o16, 2, ph[:hb], w["g16"], None, KAPPA, 0.0, 0, 0, t16), 50)
+    row("Mhat_wilson_q16_12 (2 launches: hop, hop+xpay)", ms, 2 * (52 + 192 + 52) + 52, 2 * 1320)
+    ms = gpu_time_ms(lambda: c.dslash_half(o16, 2, ph[:hb], w["g16"], w["c16"], KAPPA, CSW, 0, 0, t16), 50)
+    row("Mhat_clover_q16_12 (2 launches)", ms, 2 * (52 + 192 + 148 + 52) + 52, 2 * 1320 + 2 * 504)
     # fused BLAS-1, one-parity fp32 vectors (100 MB each; 4 distinct arrays > L2)
     x, y, p, q = (torch.randn(h, device="cuda", dtype=torch.float32) for _ in range(4))
     row("axpy_fp32", gpu_time_ms(lambda: c.axpy(1e-3, x, y), 50), 288, 48)
@@ -291,8 +301,10 @@ def solver_table(c, w):
     x = torch.empty_like(b)
     out = {}
     c.ensure_workspace(c.workspace_bytes(dims, 8))
-    for name, lo in (("mixed_cg_fp32_12/fp64_18", True), ("cg_fp64_18", False)):
-        if lo:
+    for name, lo in (("mixed_cg_q16_12/fp64_18", 2), ("mixed_cg_fp32_12/fp64_18", 1), ("cg_fp64_18", 0)):
+        if lo == 2:
+            c.set_operator(w["g64"], w["g16"], w["c64"], w["c16"], KAPPA, CSW, 0, 0.1)
+        elif lo:
             c.set_operator(w["g64"], w["g32"], w["c64"], w["c32"], KAPPA, CSW, 0, 0.1)
         else:
             c.set_operator(w["g64"], None, w["c64"], None, KAPPA, CSW, 0)
@@ -375,17 +387,20 @@ def config_table(c, peak, config4):
             c.ensure_workspace(2 * nb * V * 24 * 4)
             c.cheb_apply_multi(y, v, nb, g, kappa, coeff[:4], scale)
             torch.cuda.synchronize()
+            sampler = ClockSampler(torch.cuda.current_device())
+            sampler.start()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
             for _ in range(nvec // nb):
                 c.cheb_apply_multi(y, v, nb, g, kappa, coeff, scale)
             e1.record(); e1.synchronize()
+            clk = sampler.stop()
             sec = e0.elapsed_time(e1) * 1e-3
             per_sv = 480.0 + 384.0 / nb       # in + z + b_{k+2} + v + out = 5 x 96 B, links 384 B / nb
             byts = per_sv * (V // 2) * nvec * 100 * 2
             res["%d vector(s) per launch" % nb] = {
                 "seconds_12vec_deg100": round(sec, 4), "GFLOP/s": round(HOP_FLOP * (V // 2) * nvec * 200 / sec * 1e-9, 1),
-                "GB/s": round(byts / sec * 1e-9, 1), "frac": round(byts / sec * 1e-9 / peak, 4), "B/site-vector": per_sv}
+                "GB/s": round(byts / sec * 1e-9, 1), "frac": round(byts / sec * 1e-9 / peak, 4), "B/site-vector": per_sv, "clocks": clk}
             del v, y
         res["note"] = "Clenshaw recurrence, gamma5 and the coefficient term fused in the hop epilogue (2 launches per degree)"
         out["config4_chebyshev_48x96_fp32_12vec_deg100"] = res

@@ -20,10 +20,35 @@ constexpr size_t HALF_SPINOR_BYTES = 52;  /* per site */
 constexpr size_t HALF_LINK_BYTES = 24;
 constexpr size_t HALF_CLOVER_BYTES = 148;
 
+/* (float)code without I2F (an XU instruction, 16 lanes/clk/SM): code + 32768 in the low
+ * mantissa bits of 2^23 is the float 2^23 + 32768 + code; the subtraction is exact. */
+__device__ __forceinline__ void half_int2(int w, float& lo, float& hi)
+{
+    const unsigned x = (unsigned)w ^ 0x80008000u;
+#ifdef QCD_HALF_NO_F32X2
+    lo = __uint_as_float(__byte_perm(x, 0x4B00u, 0x5410)) - 8421376.0f;
+    hi = __uint_as_float(__byte_perm(x, 0x4B00u, 0x5432)) - 8421376.0f;
+#else
+    /* both halves in one packed add (sm_100 add.f32x2: one issue slot for two lanes) */
+    unsigned long long p, m, r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(p) : "r"(__byte_perm(x, 0x4B00u, 0x5410)), "r"(__byte_perm(x, 0x4B00u, 0x5432)));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(m) : "f"(-8421376.0f));
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(p), "l"(m));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(r));
+#endif
+}
+__device__ __forceinline__ void half_int8(const int4& w, float* o)
+{
+    half_int2(w.x, o[0], o[1]);
+    half_int2(w.y, o[2], o[3]);
+    half_int2(w.z, o[4], o[5]);
+    half_int2(w.w, o[6], o[7]);
+}
 __device__ __forceinline__ void half_unpack2(int w, float d, float& lo, float& hi)
 {
-    lo = (float)(short)(w & 0xffff) * d;
-    hi = (float)(w >> 16) * d;
+    half_int2(w, lo, hi);
+    lo *= d;
+    hi *= d;
 }
 __device__ __forceinline__ void half_unpack8(const int4& w, float d, float* o)
 {
@@ -31,6 +56,21 @@ __device__ __forceinline__ void half_unpack8(const int4& w, float d, float* o)
     half_unpack2(w.y, d, o[2], o[3]);
     half_unpack2(w.z, d, o[4], o[5]);
     half_unpack2(w.w, d, o[6], o[7]);
+}
+/* rintf(v * scale) for |v * scale| < 2^22 without F2I: adding 1.5 * 2^23 rounds to the nearest
+ * (even) integer and leaves its two's complement in the low mantissa bits.  The product is
+ * rounded to fp32 first (no fma), as the format's definition has it.  No clamp: callers
+ * guarantee |v| * scale <= 32767 (scale = 32767 / max|v|). */
+__device__ __forceinline__ int half_pack2_fast(float lo, float hi, float scale)
+{
+    const unsigned a = __float_as_uint(__fadd_rn(__fmul_rn(lo, scale), 12582912.0f));
+    const unsigned b = __float_as_uint(__fadd_rn(__fmul_rn(hi, scale), 12582912.0f));
+    return (int)__byte_perm(a, b, 0x5410);
+}
+__device__ __forceinline__ int4 half_pack8_fast(const float* v, float scale)
+{
+    return make_int4(half_pack2_fast(v[0], v[1], scale), half_pack2_fast(v[2], v[3], scale),
+                     half_pack2_fast(v[4], v[5], scale), half_pack2_fast(v[6], v[7], scale));
 }
 __device__ __forceinline__ int half_code(float v, float scale)
 {
@@ -50,13 +90,24 @@ __device__ __forceinline__ int4 half_pack8(const float* v, float scale)
 struct HalfSpinor {
     const unsigned char* block;
     size_t Vh;
-    __device__ __forceinline__ void load(float (&s)[24], int idx) const
+    /* the stored values, bit for bit: code * (norm / 32767) */
+    __device__ __forceinline__ void load_values(float (&s)[24], int idx) const
     {
         const int4* q = reinterpret_cast<const int4*>(block) + idx;
         const float n = __ldg(reinterpret_cast<const float*>(block + Vh * 48) + idx);
         const float d = __fdiv_rn(n, 32767.0f);
 #pragma unroll
         for (int c = 0; c < 3; c++) half_unpack8(__ldg(q + (size_t)c * Vh), d, &s[8 * c]);
+    }
+    /* the codes as floats; returns the factor norm / 32767 still to be applied (the hop applies
+     * it once to the colour-multiplied half spinor: 12 multiplications instead of 24) */
+    __device__ __forceinline__ float load(float (&s)[24], int idx) const
+    {
+        const int4* q = reinterpret_cast<const int4*>(block) + idx;
+        const float n = __ldg(reinterpret_cast<const float*>(block + Vh * 48) + idx);
+#pragma unroll
+        for (int c = 0; c < 3; c++) half_int8(__ldg(q + (size_t)c * Vh), &s[8 * c]);
+        return __fdiv_rn(n, 32767.0f);
     }
 };
 
@@ -68,7 +119,7 @@ __device__ __forceinline__ void half_store_spinor(unsigned char* block, size_t V
     const float scale = n > 0.f ? __fdiv_rn(32767.0f, n) : 0.f;
     int4* q = reinterpret_cast<int4*>(block) + idx;
 #pragma unroll
-    for (int c = 0; c < 3; c++) q[(size_t)c * Vh] = half_pack8(&v[8 * c], scale);
+    for (int c = 0; c < 3; c++) q[(size_t)c * Vh] = half_pack8_fast(&v[8 * c], scale);
     reinterpret_cast<float*>(block + Vh * 48)[idx] = n;
 }
 
@@ -77,17 +128,22 @@ struct HalfLinks {
     size_t gblock; /* bytes per (mu, parity) block */
     size_t Vh;
     int parity;
-    template <int MU, int DIR> __device__ __forceinline__ void get(float (&u)[18], int cb, int nb_cb) const
+    /* rows 0,1 as codes (scale 32767), row 2 = conj(row0 x row1) / 32767 on the same scale;
+     * returns the factor 1/32767 still to be applied */
+    template <int MU, int DIR> __device__ __forceinline__ float get(float (&u)[18], int cb, int nb_cb) const
     {
         const unsigned char* blk = gauge + (size_t)(2 * MU + (DIR > 0 ? parity : 1 - parity)) * gblock;
         const size_t i = (size_t)(DIR > 0 ? cb : nb_cb);
         const int4 a = __ldg(reinterpret_cast<const int4*>(blk) + i);
         const int2 b = __ldg(reinterpret_cast<const int2*>(blk + Vh * 16) + i);
         const float d = 1.0f / 32767.0f;
-        half_unpack8(a, d, &u[0]);
-        half_unpack2(b.x, d, u[8], u[9]);
-        half_unpack2(b.y, d, u[10], u[11]);
+        half_int8(a, &u[0]);
+        half_int2(b.x, u[8], u[9]);
+        half_int2(b.y, u[10], u[11]);
         reconstruct_row2<float>(u);
+#pragma unroll
+        for (int k = 12; k < 18; k++) u[k] *= d;
+        return d;
     }
 };
 

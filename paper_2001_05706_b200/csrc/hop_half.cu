@@ -8,6 +8,7 @@
  */
 #include "half_device.cuh"
 #include "hop_kernel.cuh"
+#include "packed_math.cuh"
 
 namespace {
 
@@ -33,46 +34,233 @@ __device__ __forceinline__ void half_clover_apply(float (&o)[24], const unsigned
     }
 }
 
-template <int DAG, int MODE, int OUT_F32>
-__global__ void __launch_bounds__(128, 4) hop_half_kernel(const HalfHopArgs A)
+#ifndef HOP_MINBLOCKS_HALF
+#define HOP_MINBLOCKS_HALF 8 /* blocks of 64 threads = 128 sites; swept with the depth on B200 (Wilson Mhat, 2 launches):
+                              (depth 1, 8 blocks) 213 us, (1,6) 223, (2,6) 223, (2,5) 223, (3,4) 231, (2,4) 248 */
+#endif
+#ifndef HOP_HALF_DEPTH
+#define HOP_HALF_DEPTH 1 /* directions whose loads are in flight ahead of the arithmetic */
+#endif
+
+/* The undecoded words of one direction: neighbour spinor (3 x int4 + norm) and link (int4 + int2),
+ * 19 registers.  The 16-bit kernel moves half the bytes of the fp32 one per load instruction, so
+ * it needs more loads in flight to cover the same DRAM latency: the loads of HOP_HALF_DEPTH
+ * directions are issued before the first one is decoded, and each slot is refilled as soon
+ * as it has been consumed (ncu before this: 45 % of the stall samples were long-scoreboard
+ * waits at the first use of each direction's data). */
+struct HalfRaw {
+    int4 q0, q1, q2, la;
+    int2 lb;
+    float n;
+};
+
+template <int MU, int DIR>
+__device__ __forceinline__ void half_load_raw(HalfRaw& r, const HalfHopArgs& A, size_t Vh, int cb, int nb_cb)
 {
-    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
-    if (cb >= A.geo.Vh) return;
+    const int4* q = reinterpret_cast<const int4*>(A.in) + nb_cb;
+    r.q0 = __ldg(q);
+    r.q1 = __ldg(q + Vh);
+    r.q2 = __ldg(q + 2 * Vh);
+    r.n = __ldg(reinterpret_cast<const float*>(A.in + Vh * 48) + nb_cb);
+    const unsigned char* blk = A.gauge + (size_t)(2 * MU + (DIR > 0 ? A.parity : 1 - A.parity)) * A.gblock;
+    const size_t i = (size_t)(DIR > 0 ? cb : nb_cb);
+    r.la = __ldg(reinterpret_cast<const int4*>(blk) + i);
+    r.lb = __ldg(reinterpret_cast<const int2*>(blk + Vh * 16) + i);
+}
+
+/* ---- two sites per thread on packed fp32 pairs (packed_math.cuh) ------------------------------
+ * lane A = site cbA, lane B = site cbB.  A decoded code needs one PRMT whichever register it
+ * lands in, so pairing the two sites' values costs nothing; every arithmetic instruction then
+ * serves both sites. */
+__device__ __forceinline__ void half_int2x2(int wa, int wb, f2& lo, f2& hi)
+{
+    const unsigned xa = (unsigned)wa ^ 0x80008000u, xb = (unsigned)wb ^ 0x80008000u;
+    const f2 m = f2_set1(8421376.0f);
+    lo = f2_bits(__byte_perm(xa, 0x4B00u, 0x5410), __byte_perm(xb, 0x4B00u, 0x5410)) - m;
+    hi = f2_bits(__byte_perm(xa, 0x4B00u, 0x5432), __byte_perm(xb, 0x4B00u, 0x5432)) - m;
+}
+__device__ __forceinline__ void half_int8x2(const int4& a, const int4& b, f2* o)
+{
+    half_int2x2(a.x, b.x, o[0], o[1]);
+    half_int2x2(a.y, b.y, o[2], o[3]);
+    half_int2x2(a.z, b.z, o[4], o[5]);
+    half_int2x2(a.w, b.w, o[6], o[7]);
+}
+
+template <int MU, int DIR, int SG>
+__device__ __forceinline__ void half_compute_raw2(f2 (&acc)[24], const HalfRaw& ra, const HalfRaw& rb, f2 sign)
+{
+    f2 s[24], u[18], h[12], w[12];
+    half_int8x2(ra.q0, rb.q0, &s[0]);
+    half_int8x2(ra.q1, rb.q1, &s[8]);
+    half_int8x2(ra.q2, rb.q2, &s[16]);
+    half_int8x2(ra.la, rb.la, &u[0]);
+    half_int2x2(ra.lb.x, rb.lb.x, u[8], u[9]);
+    half_int2x2(ra.lb.y, rb.lb.y, u[10], u[11]);
+    const f2 d = f2_set1(1.0f / 32767.0f);
+    reconstruct_row2_2(u, d);
+    project2<MU, SG>(h, s);
+    /* codes -> values once, on the colour-multiplied half spinor: (norm / 32767) * (1 / 32767) */
+    const f2 scale = sign * f2_make(__fdiv_rn(ra.n, 32767.0f), __fdiv_rn(rb.n, 32767.0f)) * d;
+    colour_mul2<(DIR < 0)>(w, u, h, scale);
+    reconstruct_add2<MU, SG>(acc, w);
+}
+
+/* the stored values code * (norm / 32767) of the two sites' spinors */
+__device__ __forceinline__ void half_load_values2(f2 (&v)[24], const unsigned char* block, size_t Vh, int ia, int ib)
+{
+    const int4* q = reinterpret_cast<const int4*>(block);
+    const float* nrm = reinterpret_cast<const float*>(block + Vh * 48);
+    const f2 d = f2_make(__fdiv_rn(__ldg(nrm + ia), 32767.0f), __fdiv_rn(__ldg(nrm + ib), 32767.0f));
+#pragma unroll
+    for (int c = 0; c < 3; c++) half_int8x2(__ldg(q + (size_t)c * Vh + ia), __ldg(q + (size_t)c * Vh + ib), &v[8 * c]);
+#pragma unroll
+    for (int k = 0; k < 24; k++) v[k] = v[k] * d;
+}
+
+__device__ __forceinline__ void half_clover_apply2(f2 (&o)[24], const unsigned char* clov, size_t Vh, int ia, int ib, const f2 (&v)[24])
+{
+    const int4* q = reinterpret_cast<const int4*>(clov);
+    const float* nrm = reinterpret_cast<const float*>(clov + Vh * 144);
+    const f2 d = f2_make(__fdiv_rn(__ldg(nrm + ia), 32767.0f), __fdiv_rn(__ldg(nrm + ib), 32767.0f));
+#pragma unroll
+    for (int b = 0; b < 2; b++) {
+        f2 t[40];
+#pragma unroll
+        for (int k = 0; k < 5; k++)
+            half_int8x2(__ldg(q + (size_t)(4 * b + k) * Vh + ia), __ldg(q + (size_t)(4 * b + k) * Vh + ib), &t[8 * k]);
+        /* block 1 starts at code 36 = chunk 4, offset 4; the site's scale multiplies the 12 results */
+        clover_block_apply2(&o[12 * b], &t[4 * b], &v[12 * b]);
+#pragma unroll
+        for (int k = 0; k < 12; k++) o[12 * b + k] = o[12 * b + k] * d;
+    }
+}
+
+/* 16-bit store of one lane (site idx); codes by the rule of half_store_spinor, computed packed */
+__device__ __forceinline__ void half_store2(unsigned char* block, size_t Vh, int ia, int ib, bool store_b, const f2 (&v)[24])
+{
+    float na = 0.f, nb = 0.f;
+#pragma unroll
+    for (int k = 0; k < 24; k++) {
+        float x, y;
+        f2_get(v[k], x, y);
+        na = fmaxf(na, fabsf(x));
+        nb = fmaxf(nb, fabsf(y));
+    }
+    const f2 scale = f2_make(na > 0.f ? __fdiv_rn(32767.0f, na) : 0.f, nb > 0.f ? __fdiv_rn(32767.0f, nb) : 0.f);
+    const f2 magic = f2_set1(12582912.0f);
+    unsigned ca[24], cb[24];
+#pragma unroll
+    for (int k = 0; k < 24; k++) f2_get_bits(v[k] * scale + magic, ca[k], cb[k]);
+    int4* q = reinterpret_cast<int4*>(block);
+    float* nrm = reinterpret_cast<float*>(block + Vh * 48);
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int k = 8 * c;
+        q[(size_t)c * Vh + ia] = make_int4((int)__byte_perm(ca[k], ca[k + 1], 0x5410), (int)__byte_perm(ca[k + 2], ca[k + 3], 0x5410),
+                                           (int)__byte_perm(ca[k + 4], ca[k + 5], 0x5410), (int)__byte_perm(ca[k + 6], ca[k + 7], 0x5410));
+        if (store_b)
+            q[(size_t)c * Vh + ib] = make_int4((int)__byte_perm(cb[k], cb[k + 1], 0x5410), (int)__byte_perm(cb[k + 2], cb[k + 3], 0x5410),
+                                               (int)__byte_perm(cb[k + 4], cb[k + 5], 0x5410), (int)__byte_perm(cb[k + 6], cb[k + 7], 0x5410));
+    }
+    nrm[ia] = na;
+    if (store_b) nrm[ib] = nb;
+}
+
+#define HALF_LOAD(k, MU, DIR, NB)                                          \
+    do {                                                                   \
+        half_load_raw<MU, DIR>(rawa[(k) % D], A, Vh, cba, na.NB);          \
+        half_load_raw<MU, DIR>(rawb[(k) % D], A, Vh, cbb, nbb.NB);         \
+    } while (0)
+#define HALF_COMP(k, MU, DIR, SG, SIGN) half_compute_raw2<MU, DIR, SG>(acc, rawa[(k) % D], rawb[(k) % D], SIGN)
+
+template <int DAG, int MODE, int OUT_F32>
+__global__ void __launch_bounds__(64, HOP_MINBLOCKS_HALF) hop_half_kernel(const HalfHopArgs A)
+{
+    /* a block of 64 threads works on 128 consecutive sites: thread t on base + t and base + 64 + t */
+    const int cba = blockIdx.x * 128 + threadIdx.x;
+    if (cba >= A.geo.Vh) return;
+    const bool has_b = cba + 64 < A.geo.Vh;
+    const int cbb = has_b ? cba + 64 : cba; /* ragged tail: lane B repeats lane A and is not stored */
     const size_t Vh = (size_t)A.geo.Vh;
-    const Neighbours<float> nb(A.geo, cb, A.parity, A.tb);
-    const HalfLinks L = {A.gauge, A.gblock, Vh, A.parity};
-    const HalfSpinor src = {A.in, Vh};
-    float acc[24];
-    hop_site<float, DAG>(acc, L, src, cb, nb);
+    const Neighbours<float> na(A.geo, cba, A.parity, A.tb), nbb(A.geo, cbb, A.parity, A.tb);
+    constexpr int SF = DAG ? +1 : -1; /* forward hop carries (1 - g_mu), the adjoint swaps (O4) */
+    constexpr int SB = DAG ? -1 : +1;
+    constexpr int D = HOP_HALF_DEPTH;
+    const f2 one = f2_set1(1.f);
+    f2 acc[24];
+#pragma unroll
+    for (int i = 0; i < 24; i++) acc[i].v = 0ull;
+    HalfRaw rawa[D], rawb[D];
+    /* direction k: 0 x+, 1 x-, 2 y+, 3 y-, 4 z+, 5 z-, 6 t+, 7 t-; load k + D follows compute k */
+    if (0 < D) HALF_LOAD(0, 0, +1, xp);
+    if (1 < D) HALF_LOAD(1, 0, -1, xm);
+    if (2 < D) HALF_LOAD(2, 1, +1, yp);
+    if (3 < D) HALF_LOAD(3, 1, -1, ym);
+    HALF_COMP(0, 0, +1, SF, one);
+    if (D == 1) HALF_LOAD(1, 0, -1, xm);
+    if (D == 2) HALF_LOAD(2, 1, +1, yp);
+    if (D == 3) HALF_LOAD(3, 1, -1, ym);
+    if (D == 4) HALF_LOAD(4, 2, +1, zp);
+    HALF_COMP(1, 0, -1, SB, one);
+    if (D == 1) HALF_LOAD(2, 1, +1, yp);
+    if (D == 2) HALF_LOAD(3, 1, -1, ym);
+    if (D == 3) HALF_LOAD(4, 2, +1, zp);
+    if (D == 4) HALF_LOAD(5, 2, -1, zm);
+    HALF_COMP(2, 1, +1, SF, one);
+    if (D == 1) HALF_LOAD(3, 1, -1, ym);
+    if (D == 2) HALF_LOAD(4, 2, +1, zp);
+    if (D == 3) HALF_LOAD(5, 2, -1, zm);
+    if (D == 4) HALF_LOAD(6, 3, +1, tp);
+    HALF_COMP(3, 1, -1, SB, one);
+    if (D == 1) HALF_LOAD(4, 2, +1, zp);
+    if (D == 2) HALF_LOAD(5, 2, -1, zm);
+    if (D == 3) HALF_LOAD(6, 3, +1, tp);
+    if (D == 4) HALF_LOAD(7, 3, -1, tm);
+    HALF_COMP(4, 2, +1, SF, one);
+    if (D == 1) HALF_LOAD(5, 2, -1, zm);
+    if (D == 2) HALF_LOAD(6, 3, +1, tp);
+    if (D == 3) HALF_LOAD(7, 3, -1, tm);
+    HALF_COMP(5, 2, -1, SB, one);
+    if (D == 1) HALF_LOAD(6, 3, +1, tp);
+    if (D == 2) HALF_LOAD(7, 3, -1, tm);
+    HALF_COMP(6, 3, +1, SF, f2_make(na.sgn_tp, nbb.sgn_tp));
+    if (D == 1) HALF_LOAD(7, 3, -1, tm);
+    HALF_COMP(7, 3, -1, SB, f2_make(na.sgn_tm, nbb.sgn_tm));
 
     if (MODE == HOP_XPAY || MODE == HOP_CLOVER_Z) {
-        const HalfSpinor zs = {A.z, Vh};
-        float zz[24];
-        zs.load(zz, cb);
+        f2 zz[24];
+        half_load_values2(zz, A.z, Vh, cba, cbb);
+        const f2 ca = f2_set1(A.a), cb = f2_set1(A.b);
         if (MODE == HOP_CLOVER_Z) {
-            float az[24];
-            half_clover_apply(az, A.clover, Vh, (size_t)cb, zz);
+            f2 az[24];
+            half_clover_apply2(az, A.clover, Vh, cba, cbb, zz);
 #pragma unroll
-            for (int i = 0; i < 24; i++) acc[i] = A.a * az[i] + A.b * acc[i];
+            for (int i = 0; i < 24; i++) acc[i] = f2_fma(ca, az[i], cb * acc[i]);
         } else {
 #pragma unroll
-            for (int i = 0; i < 24; i++) acc[i] = A.a * zz[i] + A.b * acc[i];
+            for (int i = 0; i < 24; i++) acc[i] = f2_fma(ca, zz[i], cb * acc[i]);
         }
     } else if (MODE == HOP_CLOVER_OUT) {
-        float o[24];
-        half_clover_apply(o, A.clover, Vh, (size_t)cb, acc);
+        f2 o[24];
+        half_clover_apply2(o, A.clover, Vh, cba, cbb, acc);
 #pragma unroll
         for (int i = 0; i < 24; i++) acc[i] = o[i];
     }
-    if (OUT_F32)
-        store_planes<float, 24>(reinterpret_cast<float*>(A.out), Vh, (size_t)cb, acc);
-    else
-        half_store_spinor(A.out, Vh, (size_t)cb, acc);
+    if (OUT_F32) {
+        float va[24], vb[24];
+#pragma unroll
+        for (int i = 0; i < 24; i++) f2_get(acc[i], va[i], vb[i]);
+        store_planes<float, 24>(reinterpret_cast<float*>(A.out), Vh, (size_t)cba, va);
+        if (has_b) store_planes<float, 24>(reinterpret_cast<float*>(A.out), Vh, (size_t)cbb, vb);
+    } else {
+        half_store2(A.out, Vh, cba, cbb, has_b, acc);
+    }
 }
 
 template <int DAG, int MODE> cudaError_t launch_mode(const HalfHopArgs& A, int out_f32, cudaStream_t st)
 {
-    const int threads = 128, blocks = (A.geo.Vh + threads - 1) / threads;
+    const int threads = 64, blocks = (A.geo.Vh + 127) / 128;
     if (out_f32) hop_half_kernel<DAG, MODE, 1><<<blocks, threads, 0, st>>>(A);
     else hop_half_kernel<DAG, MODE, 0><<<blocks, threads, 0, st>>>(A);
     return cudaGetLastError();
@@ -100,7 +288,7 @@ template <int TO_HALF> __global__ void half_convert_kernel(unsigned char* half, 
         half_store_spinor(half + blk * HALF_SPINOR_BYTES * Vh, Vh, cb, v);
     } else {
         const HalfSpinor s = {half + blk * HALF_SPINOR_BYTES * Vh, Vh};
-        s.load(v, (int)cb);
+        s.load_values(v, (int)cb);
         store_planes<float, 24>(f32 + blk * 24 * Vh, Vh, cb, v);
     }
 }

@@ -40,7 +40,14 @@ template <typename T> struct HopArgs {
 template <typename T> struct PlaneSpinor {
     const T* base;
     size_t Vh;
-    __device__ __forceinline__ void load(T (&s)[24], int idx) const { load_planes<T, 24>(s, base, Vh, (size_t)idx); }
+    /* load() and Links::get() return the factor their values still have to be multiplied by
+     * (1 here; the 16-bit sources return their scale so that it is applied once, to the
+     * colour-multiplied half spinor, instead of to every decoded value) */
+    __device__ __forceinline__ T load(T (&s)[24], int idx) const
+    {
+        load_planes<T, 24>(s, base, Vh, (size_t)idx);
+        return (T)1;
+    }
 };
 
 /* ---- where a direction's link comes from ------------------------------------------- */
@@ -48,12 +55,13 @@ template <typename T, int RECON> struct GlobalLinks {
     const T* gauge;
     size_t gblock, Vh;
     int parity;
-    template <int MU, int DIR> __device__ __forceinline__ void get(T (&u)[18], int cb, int nb_cb) const
+    template <int MU, int DIR> __device__ __forceinline__ T get(T (&u)[18], int cb, int nb_cb) const
     {
         if (DIR > 0)
             load_link<T, RECON>(u, gauge + (size_t)(2 * MU + parity) * gblock, Vh, (size_t)cb);
         else
             load_link<T, RECON>(u, gauge + (size_t)(2 * MU + (1 - parity)) * gblock, Vh, (size_t)nb_cb);
+        return (T)1;
     }
 };
 
@@ -74,7 +82,7 @@ template <typename T, int RECON> struct SmemLinks {
 #pragma unroll
         for (int c = 0; c < NCH; c++) slot[(d * NCH + c) * 128] = vec_make(&r[c * Vec<T>::reals]);
     }
-    template <int MU, int DIR> __device__ __forceinline__ void get(T (&u)[18], int, int) const
+    template <int MU, int DIR> __device__ __forceinline__ T get(T (&u)[18], int, int) const
     {
         constexpr int d = 2 * MU + (DIR < 0 ? 1 : 0);
         T r[NCH * Vec<T>::reals];
@@ -83,6 +91,7 @@ template <typename T, int RECON> struct SmemLinks {
 #pragma unroll
         for (int i = 0; i < RECON; i++) u[i] = r[i];
         if (RECON == 12) reconstruct_row2<T>(u);
+        return (T)1;
     }
 };
 
@@ -180,10 +189,10 @@ template <typename T, int MU, int DIR, int SG, typename Links, typename Src>
 __device__ __forceinline__ void hop_dir(T (&acc)[24], const Links& L, const Src& in, int cb, int nb_cb, T sign)
 {
     T s[24], u[18], h[12], w[12];
-    in.load(s, nb_cb);
-    L.template get<MU, DIR>(u, cb, nb_cb);
+    const T fs = in.load(s, nb_cb);
+    const T fu = L.template get<MU, DIR>(u, cb, nb_cb);
     project<T, MU, SG>(h, s);
-    colour_mul<T, (DIR < 0)>(w, u, h, sign);
+    colour_mul<T, (DIR < 0)>(w, u, h, sign * fs * fu);
     reconstruct_add<T, MU, SG>(acc, w);
 }
 
@@ -332,6 +341,37 @@ __device__ __forceinline__ void cheb_vector(const HopArgs<T>& A, const Links& L,
     store_planes_cs<T, 24>(A.out + off, Vh, (size_t)cb, acc);
 }
 
+#ifndef HOP_CHEB_PREFETCH
+#define HOP_CHEB_PREFETCH 1 /* swept on B200 (48^3x96, 12 vectors): 0 1.40 s, 1 1.35 s, 2 1.47 s, 4 1.44 s, 6 1.57 s, 15 1.84 s */
+#endif
+/* Everything vector j of the multi-rhs loop will read, requested into L2 one vector ahead: its
+ * eight neighbour spinors and its own-site streams.  ncu before this: 59 % of the stall samples
+ * were long-scoreboard waits, the largest at the first use of direction 0 and of z / tm / v,
+ * whose loads the compiler cannot hoist across the vector loop.  Only the own-site streams of the
+ * current vector pay (bit 0); prefetching neighbours a vector ahead costs more than it hides. */
+template <typename T, int WHAT>
+__device__ __forceinline__ void cheb_prefetch(const HopArgs<T>& A, size_t off, size_t Vh, int cb, const Neighbours<T>& nb)
+{
+    if (WHAT & 2) {
+        const T* in = A.in + off;
+        prefetch_planes_l2<T, 24>(in, Vh, (size_t)nb.xp);
+        prefetch_planes_l2<T, 24>(in, Vh, (size_t)nb.xm);
+        if (WHAT & 8) {
+            prefetch_planes_l2<T, 24>(in, Vh, (size_t)nb.yp);
+            prefetch_planes_l2<T, 24>(in, Vh, (size_t)nb.ym);
+            prefetch_planes_l2<T, 24>(in, Vh, (size_t)nb.zp);
+            prefetch_planes_l2<T, 24>(in, Vh, (size_t)nb.zm);
+            prefetch_planes_l2<T, 24>(in, Vh, (size_t)nb.tp);
+            prefetch_planes_l2<T, 24>(in, Vh, (size_t)nb.tm);
+        }
+    }
+    if (WHAT & 1) {
+        prefetch_planes_l2<T, 24>(A.z + off, Vh, (size_t)cb);
+        if (A.c3 != (T)0) prefetch_planes_l2<T, 24>(A.v + off, Vh, (size_t)cb);
+        if (A.c2 != (T)0) prefetch_planes_l2<T, 24>(A.tm + off, Vh, (size_t)cb);
+    }
+}
+
 /* STAGE = 1: nvec > 1, links parked in shared memory; STAGE = 0: one vector, links straight from HBM */
 template <typename T, int RECON, int STAGE>
 __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_cheb_mrhs_kernel(const HopArgs<T> A)
@@ -360,6 +400,7 @@ __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_cheb_mrhs_k
         return;
     }
     const SmemLinks<T, RECON> S = {reinterpret_cast<V*>(smem_raw) + threadIdx.x};
+    if (HOP_CHEB_PREFETCH & 4) cheb_prefetch<T, 1>(A, 0, Vh, cb, nb);
     {
         T u[18];
         G.template get<0, +1>(u, cb, nb.xp); S.template put<0, +1>(u);
@@ -371,7 +412,14 @@ __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_cheb_mrhs_k
         G.template get<3, +1>(u, cb, nb.tp); S.template put<3, +1>(u);
         G.template get<3, -1>(u, cb, nb.tm); S.template put<3, -1>(u);
     }
-    for (int j = 0; j < A.nvec; j++) cheb_vector<T>(A, S, (size_t)j * A.vstride, Vh, cb, nb);
+    for (int j = 0; j < A.nvec; j++) {
+        /* bit 0: own-site streams of this vector now; bit 2: of the next vector instead;
+         * bit 1: x neighbours of the next vector; bit 3: all its neighbours */
+        if ((HOP_CHEB_PREFETCH & 5) == 1) cheb_prefetch<T, 1>(A, (size_t)j * A.vstride, Vh, cb, nb);
+        if ((HOP_CHEB_PREFETCH & 4) && j + 1 < A.nvec) cheb_prefetch<T, 1>(A, (size_t)(j + 1) * A.vstride, Vh, cb, nb);
+        if ((HOP_CHEB_PREFETCH & 2) && j + 1 < A.nvec) cheb_prefetch<T, (HOP_CHEB_PREFETCH & 10)>(A, (size_t)(j + 1) * A.vstride, Vh, cb, nb);
+        cheb_vector<T>(A, S, (size_t)j * A.vstride, Vh, cb, nb);
+    }
 }
 
 template <typename T, int RECON> static cudaError_t hop_cheb_launch(const HopArgs<T>& A, cudaStream_t st)

@@ -73,6 +73,16 @@ __device__ __forceinline__ void load_planes_cs(T (&d)[NREAL], const T* base, siz
         vec_get(v, &d[c * Vec<T>::reals]);
     }
 }
+/* L2 prefetch of the NREAL reals of site idx (one line request per 128-bit plane, no register
+ * is tied up): used where a thread knows, a whole vector ahead, what it will read next */
+template <typename T, int NREAL>
+__device__ __forceinline__ void prefetch_planes_l2(const T* base, size_t stride, size_t idx)
+{
+    typedef typename Vec<T>::type V;
+    const V* p = reinterpret_cast<const V*>(base) + idx;
+#pragma unroll
+    for (int c = 0; c < NREAL / Vec<T>::reals; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(p + (size_t)c * stride));
+}
 template <typename T, int NREAL>
 __device__ __forceinline__ void store_planes_cs(T* base, size_t stride, size_t idx, const T (&d)[NREAL])
 {

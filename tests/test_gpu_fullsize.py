@@ -223,3 +223,61 @@ def test_config4_chebyshev_48x96_reduced_degree_full_size():
         got = c.spinor_unpack(y[i * n:(i + 1) * n].contiguous(), dims).cpu().numpy()
         assert relerr(got, want) <= 2e-6
     c.set_workspace(None)
+
+
+# ---- 16-bit storage at full size (reading H1) --------------------------------
+def test_half_wilson_full_operator_sampled_sites_32x64(world):
+    """D = 1 - kappa H with 16-bit links and a 16-bit input spinor at 32^3 x 64 (full lattice,
+    fp32 output), compared on sampled sites with the oracle's hop on the stored-and-read-back
+    fields; the stored codes of a sampled site are compared bit for bit."""
+    c, U, psi, g, g18, cl, pin = world
+    dU = torch.from_numpy(U).cuda()
+    g16 = c.gauge_load(dU, DIMS, 2, 12, -1)
+    del dU
+    Vh = pin.numel() // 48
+    ph = c.spinor_to_half(pin, DIMS, 2)
+    out = torch.empty_like(pin)
+    c.dslash_half(out, 4, ph, g16, None, KAPPA, 0.0, 2, 0)
+    got = c.spinor_unpack(out, DIMS).cpu().numpy().astype(np.float64).reshape(-1, 4, 3, 2)
+    psi_q = orc.q16_spinor(psi.astype(np.float32)).astype(np.float64)
+    back = c.spinor_unpack(c.spinor_from_half(ph, DIMS, 2), DIMS).cpu().numpy()
+    assert np.array_equal(back, psi_q.astype(np.float32).reshape(back.shape))
+    Uq = orc.q16_links(U.astype(np.float32)).astype(np.float64)
+    for parity in (0, 1):
+        S = sample_sites(parity, 40, 21 + parity)
+        want = psi_q.reshape(-1, 4, 3, 2)[S] - KAPPA * orc.hop_sites(psi_q, Uq, DIMS, S, -1, False)
+        assert relerr(got[S], want) <= 2e-6
+    del g16
+
+
+def test_half_mixed_cg_32x64_full_size(world):
+    """configs[3] at full size with the 16-bit operator inside the reliable-update CG, against the
+    oracle running the same algorithm (half=True): iterations +-2, fp64 true residual below tol."""
+    if _host_mem_gb() < 60:
+        pytest.skip("needs ~50 GB of host memory for the oracle's dense clover fields")
+    c = ctx()
+    tol = 1e-10
+    U = inputs.tiled_gauge_field(DIMS, 0.5, 0, 16)
+    A = orc.clover_matrix(orc.field_strength(U, DIMS), DIMS, KAPPA * CSW)
+    Ainv = orc.invert_12(A)
+    par = orc.parity_mask_array(DIMS)[..., None, None, None]
+    b = inputs.spinor_field(DIMS, 0, 1) * (par == 0)
+    y_ref, st_ref = orc.cg_mixed(b, U, DIMS, KAPPA, tol, 5000, A, Ainv, -1, 0, 0.1, half=True)
+    del A, Ainv
+    dU = torch.from_numpy(U).cuda()
+    g_hi = c.gauge_load(dU, DIMS, 8, 18, -1)
+    g16 = c.gauge_load(dU, DIMS, 2, 12, -1)
+    del dU
+    c_hi = c.clover_build(g_hi, KAPPA, CSW, 8)
+    c16 = c.clover_build(g_hi, KAPPA, CSW, 2)
+    c.ensure_workspace(c.workspace_bytes(DIMS, 8))
+    c.set_operator(g_hi, g16, c_hi, c16, KAPPA, CSW, 0, 0.1)
+    pb = c.spinor_pack(torch.from_numpy(b).cuda(), DIMS)
+    h = pb.numel() // 2
+    full = torch.zeros_like(pb)
+    rc, st = c.cg_solve(full[:h], pb[:h], tol, 5000)
+    assert rc == 0 and st.converged == 1
+    assert abs(st.iters - st_ref["iters"]) <= 2
+    assert abs(st.reliable_updates - st_ref["reliable_updates"]) <= 1
+    assert st.r_true < 1.5 * tol
+    assert relerr(c.spinor_unpack(full, DIMS).cpu().numpy(), y_ref) <= 1e-8
