@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-solvers", action="store_true", help="kernel table only (for ncu passes)")
     ap.add_argument("--config4", action="store_true", help="also run the 48^3x96 Chebyshev workload (configs[4])")
+    ap.add_argument("--config4-only", action="store_true", help="only the configs[4] section (for ncu passes)")
+    ap.add_argument("--cheb-degree", type=int, default=100, help="Chebyshev degree timed in the configs[4] section")
     ap.add_argument("--table-scale", type=float, default=1.0, help="scale the iteration counts of the kernel table")
     return ap.parse_args()
 
@@ -325,52 +327,75 @@ def solver_table(c, w):
     return out
 
 
-def config_table(c, peak, config4):
+def config_table(c, peak, config4, only4=False, cheb_degree=100):
     """The other BASELINE.json configs at their full sizes (parity for each is in tests/)."""
     import torch
     from paper_2001_05706_b200 import inputs
     out = {}
-    # configs[1]: 16^3x32 fp32 even-odd Wilson, kappa 0.137, 18- and 12-real; single apply + 100-loop.
-    dims, kappa = (16, 16, 16, 32), 0.137
-    Vh = 16 * 16 * 16 * 32 // 2
-    h = Vh * 24
-    dU = torch.from_numpy(inputs.gauge_field(dims, EPS, 0)).cuda()
-    pin = c.spinor_pack(torch.from_numpy(inputs.spinor_field(dims, 0, 0)).float().cuda(), dims)
-    src, dst, tmp = pin[:h].clone(), torch.empty_like(pin[:h]), torch.empty_like(pin[:h])
-    for rec in (18, 12):
-        g = c.gauge_load(dU, dims, 4, rec, -1)
-        fn = lambda: c.dslash_ex(dst, src, g, None, kappa, 0.0, 0, 0, tmp)
-        loop_ms = gpu_time_ms(fn, 100)
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(); fn(); e1.record(); e1.synchronize()
-        flop = 2 * HOP_FLOP * Vh
-        byts = (2 * (48 + 8 * rec) + 24) * 4 * Vh
-        out["config1_wilson_eo_16x32_fp32_%d" % rec] = {
-            "single_apply_us": round(e0.elapsed_time(e1) * 1e3, 2), "loop100_us_per_apply": round(loop_ms * 1e3, 2),
-            "GFLOP/s": round(flop / (loop_ms * 1e-3) * 1e-9, 1), "GB/s": round(byts / (loop_ms * 1e-3) * 1e-9, 1),
-            "frac": round(byts / (loop_ms * 1e-3) * 1e-9 / peak, 4),
-            "note": "L2-resident (38-50 MB working set): the HBM fraction is not a roofline statement here"}
-    del dU
-    # configs[2]: 24^3x64 fp64 Wilson-clover CG, kappa 0.135, csw 1, tol 1e-10, maxiter 5000.
-    dims, kappa = (24, 24, 24, 64), 0.135
-    Vh = 24 * 24 * 24 * 64 // 2
-    h = Vh * 24
-    dU = torch.from_numpy(inputs.tiled_gauge_field(dims, EPS, 0, 16)).cuda()
-    g = c.gauge_load(dU, dims, 8, 18, -1)
-    del dU
-    cl = c.clover_build(g, kappa, CSW, 8)
-    b = c.spinor_pack(torch.from_numpy(inputs.spinor_field(dims, 0, 1)).cuda(), dims)
-    c.ensure_workspace(c.workspace_bytes(dims, 8))
-    for name, mode in (("config2_clover_cg_24x64_fp64_evenodd", 0), ("config2_clover_cg_24x64_fp64_full", 2)):
-        c.set_operator(g, None, cl, None, kappa, CSW, mode)
-        bb = b[:h].clone() if mode == 0 else b
-        x = torch.empty_like(bb)
-        c.cg_solve(x, bb, 1e-10, 5000)
-        rc, st = c.cg_solve(x, bb, 1e-10, 5000)
-        out[name] = {"seconds": round(st.seconds, 5), "iters": st.iters, "r_true": st.r_true, "rc": rc,
-                     "GFLOP/s": round(st.flops / st.seconds * 1e-9, 1), "ms_per_iter": round(st.seconds / max(st.iters, 1) * 1e3, 4)}
-    del g, cl, b
+    if not only4:
+        # configs[1]: 16^3x32 fp32 even-odd Wilson, kappa 0.137, 18- and 12-real; single apply + 100-loop.
+        dims, kappa = (16, 16, 16, 32), 0.137
+        Vh = 16 * 16 * 16 * 32 // 2
+        h = Vh * 24
+        dU = torch.from_numpy(inputs.gauge_field(dims, EPS, 0)).cuda()
+        pin = c.spinor_pack(torch.from_numpy(inputs.spinor_field(dims, 0, 0)).float().cuda(), dims)
+        src, dst, tmp = pin[:h].clone(), torch.empty_like(pin[:h]), torch.empty_like(pin[:h])
+        from paper_2001_05706_b200 import qcd
+        gs = torch.cuda.Stream()
+        cgx = qcd.Context(torch.cuda.current_device(), stream=gs)   # a ctx on a capturable side stream
+        for rec in (18, 12):
+            g = c.gauge_load(dU, dims, 4, rec, -1)
+            fn = lambda: c.dslash_ex(dst, src, g, None, kappa, 0.0, 0, 0, tmp)
+            loop_ms = gpu_time_ms(fn, 100)
+            # the same 100-apply loop captured once in a CUDA graph and replayed (SURVEY 8(d) caveat i)
+            gs.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(gs):
+                gg = cgx.gauge_load(dU, dims, 4, rec, -1)
+                cgx.dslash_ex(dst, src, gg, None, kappa, 0.0, 0, 0, tmp)
+            gs.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=gs):
+                for _ in range(100):
+                    cgx.dslash_ex(dst, src, gg, None, kappa, 0.0, 0, 0, tmp)
+            graph.replay()
+            torch.cuda.synchronize()
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record()
+            for _ in range(5):
+                graph.replay()
+            g1.record(); g1.synchronize()
+            graph_ms = g0.elapsed_time(g1) / 500.0
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record(); e1.synchronize()
+            flop = 2 * HOP_FLOP * Vh
+            byts = (2 * (48 + 8 * rec) + 24) * 4 * Vh
+            out["config1_wilson_eo_16x32_fp32_%d" % rec] = {
+                "single_apply_us": round(e0.elapsed_time(e1) * 1e3, 2), "loop100_us_per_apply": round(loop_ms * 1e3, 2),
+                "graph100_us_per_apply": round(graph_ms * 1e3, 2),
+                "GFLOP/s": round(flop / (loop_ms * 1e-3) * 1e-9, 1), "GB/s": round(byts / (loop_ms * 1e-3) * 1e-9, 1),
+                "frac": round(byts / (loop_ms * 1e-3) * 1e-9 / peak, 4),
+                "note": "L2-resident (38-50 MB working set): the HBM fraction is not a roofline statement here"}
+        del dU
+        # configs[2]: 24^3x64 fp64 Wilson-clover CG, kappa 0.135, csw 1, tol 1e-10, maxiter 5000.
+        dims, kappa = (24, 24, 24, 64), 0.135
+        Vh = 24 * 24 * 24 * 64 // 2
+        h = Vh * 24
+        dU = torch.from_numpy(inputs.tiled_gauge_field(dims, EPS, 0, 16)).cuda()
+        g = c.gauge_load(dU, dims, 8, 18, -1)
+        del dU
+        cl = c.clover_build(g, kappa, CSW, 8)
+        b = c.spinor_pack(torch.from_numpy(inputs.spinor_field(dims, 0, 1)).cuda(), dims)
+        c.ensure_workspace(c.workspace_bytes(dims, 8))
+        for name, mode in (("config2_clover_cg_24x64_fp64_evenodd", 0), ("config2_clover_cg_24x64_fp64_full", 2)):
+            c.set_operator(g, None, cl, None, kappa, CSW, mode)
+            bb = b[:h].clone() if mode == 0 else b
+            x = torch.empty_like(bb)
+            c.cg_solve(x, bb, 1e-10, 5000)
+            rc, st = c.cg_solve(x, bb, 1e-10, 5000)
+            out[name] = {"seconds": round(st.seconds, 5), "iters": st.iters, "r_true": st.r_true, "rc": rc,
+                         "GFLOP/s": round(st.flops / st.seconds * 1e-9, 1), "ms_per_iter": round(st.seconds / max(st.iters, 1) * 1e3, 4)}
+        del g, cl, b
     if config4:
         # configs[4]: degree-100 Chebyshev of H_W (kappa 0.2) on 12 Gaussian vectors, 48^3x96 fp32.
         dims, kappa, scale, nvec = (48, 48, 48, 96), 0.2, 2.6, 12
@@ -378,7 +403,7 @@ def config_table(c, peak, config4):
         dU = torch.from_numpy(inputs.tiled_gauge_field(dims, EPS, 0, 8).astype("float32")).cuda()
         g = c.gauge_load(dU, dims, 4, 12, -1)
         del dU
-        coeff = inputs.chebyshev_sign_coefficients(100)
+        coeff = inputs.chebyshev_sign_coefficients(100)[:cheb_degree + 1]
         res = {}
         for nb in (1, 12):
             v = torch.randn(nb * V * 24, device="cuda", dtype=torch.float32)
@@ -397,13 +422,14 @@ def config_table(c, peak, config4):
             clk = sampler.stop()
             sec = e0.elapsed_time(e1) * 1e-3
             per_sv = 480.0 + 384.0 / nb       # in + z + b_{k+2} + v + out = 5 x 96 B, links 384 B / nb
-            byts = per_sv * (V // 2) * nvec * 100 * 2
+            byts = per_sv * (V // 2) * nvec * cheb_degree * 2
             res["%d vector(s) per launch" % nb] = {
-                "seconds_12vec_deg100": round(sec, 4), "GFLOP/s": round(HOP_FLOP * (V // 2) * nvec * 200 / sec * 1e-9, 1),
+                "seconds_12vec_deg%d" % cheb_degree: round(sec, 4),
+                "GFLOP/s": round(HOP_FLOP * (V // 2) * nvec * 2 * cheb_degree / sec * 1e-9, 1),
                 "GB/s": round(byts / sec * 1e-9, 1), "frac": round(byts / sec * 1e-9 / peak, 4), "B/site-vector": per_sv, "clocks": clk}
             del v, y
         res["note"] = "Clenshaw recurrence, gamma5 and the coefficient term fused in the hop epilogue (2 launches per degree)"
-        out["config4_chebyshev_48x96_fp32_12vec_deg100"] = res
+        out["config4_chebyshev_48x96_fp32_12vec_deg%d" % cheb_degree] = res
     return out
 
 
@@ -444,7 +470,7 @@ def run_ours(args):
     from paper_2001_05706_b200 import qcd
     c = qcd.Context(local)
     peak, peak_src = measured_peaks()
-    full = (not args.quick) and rank == 0
+    full = (not args.quick) and rank == 0 and not args.config4_only
     w = build_workload(c, DIMS, want_hi=full)
     dims = DIMS
     Vh = dims[0] * dims[1] * dims[2] * dims[3] // 2
@@ -539,7 +565,11 @@ def run_ours(args):
             line["cg"] = solver_table(c, w)
             del w
             torch.cuda.empty_cache()
-            line["configs"] = config_table(c, peak, args.config4)
+            line["configs"] = config_table(c, peak, args.config4, cheb_degree=args.cheb_degree)
+    if args.config4_only and rank == 0:
+        del w
+        torch.cuda.empty_cache()
+        line["configs"] = config_table(c, peak, True, only4=True, cheb_degree=args.cheb_degree)
     print(json.dumps(line))
     if world > 1:
         dist.barrier()

@@ -342,13 +342,16 @@ __device__ __forceinline__ void cheb_vector(const HopArgs<T>& A, const Links& L,
 }
 
 #ifndef HOP_CHEB_PREFETCH
-#define HOP_CHEB_PREFETCH 1 /* swept on B200 (48^3x96, 12 vectors): 0 1.40 s, 1 1.35 s, 2 1.47 s, 4 1.44 s, 6 1.57 s, 15 1.84 s */
+#define HOP_CHEB_PREFETCH 1
 #endif
-/* Everything vector j of the multi-rhs loop will read, requested into L2 one vector ahead: its
- * eight neighbour spinors and its own-site streams.  ncu before this: 59 % of the stall samples
- * were long-scoreboard waits, the largest at the first use of direction 0 and of z / tm / v,
- * whose loads the compiler cannot hoist across the vector loop.  Only the own-site streams of the
- * current vector pay (bit 0); prefetching neighbours a vector ahead costs more than it hides. */
+/* Optional L2 prefetch (prefetch.global.L2, no register tied up) of what a vector of the multi-rhs
+ * loop will read: bit 0 the own-site streams z / v / tm of the current vector, bit 2 those of the
+ * next vector instead, bit 1 the x neighbours of the next vector, bit 3 all its neighbours.
+ * Motivation: 59 % of the ncu stall samples are long-scoreboard waits, the largest at the first
+ * use of direction 0 and of z / tm / v, whose loads the compiler cannot hoist across the vector
+ * loop.  Measured on B200 (48^3x96, 12 vectors, degree 100): 0 -> 1.40 s, 1 -> 1.35 s, 2 -> 1.47 s,
+ * 4 -> 1.44 s, 6 -> 1.57 s, 15 -> 1.84 s; ncu on one 12-vector launch: 6.31 ms -> 6.05 ms with bit 0,
+ * DRAM traffic unchanged (36.6 GB).  Requesting neighbours a vector ahead costs more than it hides. */
 template <typename T, int WHAT>
 __device__ __forceinline__ void cheb_prefetch(const HopArgs<T>& A, size_t off, size_t Vh, int cb, const Neighbours<T>& nb)
 {
