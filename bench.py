@@ -517,27 +517,41 @@ def run_ours(args):
                 "kernel": "hop_kernel<float,12,0,CLOVER_OUT|CLOVER_Z>", "bytes_per_launch": bytes_launch,
                 "us_per_launch": round(ms_launch * 1e3, 2)}
 
-    # ---- end to end: HOST buffers through qcd_dslash_host (H2D + Mhat + D2H every step)
+    # ---- end to end: HOST buffers through the C ABI, H2D + Mhat + D2H for every step inside the
+    # timed region.  qcd_dslash_host_batch pipelines the steps (H2D of step i+1, operator on step i,
+    # D2H of step i-1 overlap); qcd_dslash_host is the same thing one synchronous call per step.
     blk_bytes = h * 4
-    c.ensure_workspace(max(3 * blk_bytes, c._ws.numel() if c._ws is not None else 0))
-    hin = torch.empty(h, dtype=torch.float32).pin_memory()
-    hout = torch.empty(h, dtype=torch.float32).pin_memory()
-    hin.copy_(src.cpu())
-    e2e_steps = max(3, min(20, args.steps))
-    for _ in range(2):
-        c.dslash_host(hout, hin, g, cl, KAPPA, CSW, 0, 0)
+    e2e_steps = max(4, min(16, args.steps))
+    c.ensure_workspace(max(5 * blk_bytes, c._ws.numel() if c._ws is not None else 0))
+    hin = torch.empty(e2e_steps * h, dtype=torch.float32).pin_memory()
+    hout = torch.empty(e2e_steps * h, dtype=torch.float32).pin_memory()
+    hsrc = src.cpu()
+    for i in range(e2e_steps):
+        hin[i * h:(i + 1) * h].copy_(hsrc)
+    del hsrc
+    c.dslash_host_batch(hout, hin, e2e_steps, g, cl, KAPPA, CSW, 0, 0)        # warm-up (creates the copy streams)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     e0.record()
-    for _ in range(e2e_steps):
-        c.dslash_host(hout, hin, g, cl, KAPPA, CSW, 0, 0)
+    c.dslash_host_batch(hout, hin, e2e_steps, g, cl, KAPPA, CSW, 0, 0)
     e1.record()
     torch.cuda.synchronize()
     e2e_ms = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3) / e2e_steps
     e2e_ms = max_over_ranks(e2e_ms)
+    for _ in range(2):
+        c.dslash_host(hout[:h], hin[:h], g, cl, KAPPA, CSW, 0, 0)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        c.dslash_host(hout[:h], hin[:h], g, cl, KAPPA, CSW, 0, 0)
+    torch.cuda.synchronize()
+    sync_ms = max_over_ranks((time.perf_counter() - t0) * 1e3 / e2e_steps)
     e2e = {"value": round(job_value(world, step_flops(Vh), e2e_ms), 1), "unit": UNIT,
            "h2d_bytes_per_step": blk_bytes, "d2h_bytes_per_step": blk_bytes, "ms_per_step": round(e2e_ms, 4),
-           "steps": e2e_steps, "call": "qcd_dslash_host"}
+           "steps": e2e_steps, "call": "qcd_dslash_host_batch (pipelined H2D / Mhat / D2H, pinned host buffers)",
+           "one_call_per_step": {"value": round(job_value(world, step_flops(Vh), sync_ms), 1), "ms_per_step": round(sync_ms, 4),
+                                 "call": "qcd_dslash_host"}}
+    del hin, hout
 
     if rank != 0:
         if world > 1:

@@ -242,6 +242,17 @@ int qcd_hop_host(qcd_ctx* ctx, void* out_host, const void* in_host, const qcd_ga
 int qcd_dslash_host(qcd_ctx* ctx, void* out_host, const void* in_host, const qcd_gauge* g,
                     const qcd_clover* c, double kappa, double csw, int parity, int flags);
 
+/* The same for nvec HOST vectors (vector i at in_host + i * in_stride, result at out_host +
+ * i * out_stride, strides in bytes, 0 = the same buffer every time), as a three-stage pipeline:
+ * the H2D copy of vector i+1, the operator on vector i and the D2H copy of vector i-1 overlap
+ * (two copy streams owned by the ctx; PCIe is full duplex).  Host buffers should be pinned, else
+ * the copies serialise.  Needs a workspace of 4 * field + one parity block.  Returns after the
+ * last result has landed in host memory.  The kernels are qcd_dslash's: per-vector results are
+ * bit-identical to qcd_dslash_host. */
+int qcd_dslash_host_batch(qcd_ctx* ctx, void* out_host, const void* in_host, int nvec,
+                          size_t out_stride, size_t in_stride, const qcd_gauge* g, const qcd_clover* c,
+                          double kappa, double csw, int parity, int flags);
+
 /* number of kernels this library has launched on this ctx since qcd_init */
 long long qcd_launch_count(const qcd_ctx* ctx);
 

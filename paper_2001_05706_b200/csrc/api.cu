@@ -87,6 +87,16 @@ int qcd_finalize(qcd_ctx* c)
     if (c->d_ticket) cudaFree(c->d_ticket);
     if (c->d_scalar) cudaFree(c->d_scalar);
     if (c->h_scalar) cudaFreeHost(c->h_scalar);
+    if (c->pipe_ready) {
+        cudaStreamDestroy(c->s_h2d);
+        cudaStreamDestroy(c->s_d2h);
+        cudaEventDestroy(c->ev_start);
+        for (int b = 0; b < 2; b++) {
+            cudaEventDestroy(c->ev_in[b]);
+            cudaEventDestroy(c->ev_comp[b]);
+            cudaEventDestroy(c->ev_out[b]);
+        }
+    }
     free(c);
     return QCD_OK;
 }
@@ -508,6 +518,60 @@ int qcd_dslash_host(qcd_ctx* ctx, void* out_host, const void* in_host, const qcd
     int rc = qcd_dslash_ex(d_out, d_in, g, c, kappa, csw, parity, flags, d_tmp);
     if (rc) return rc;
     QCD_CHECK_CUDA(cudaMemcpyAsync(out_host, d_out, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    QCD_CHECK_CUDA(cudaStreamSynchronize(ctx->stream));
+    return QCD_OK;
+}
+
+/* nvec host vectors through the operator as a three-stage pipeline: H2D of vector i+1, the
+ * operator on vector i and D2H of vector i-1 run concurrently (PCIe is full duplex), on two
+ * copy streams of the ctx and the ctx stream, with double-buffered device input / output. */
+int qcd_dslash_host_batch(qcd_ctx* ctx, void* out_host, const void* in_host, int nvec, size_t out_stride, size_t in_stride,
+                          const qcd_gauge* g, const qcd_clover* c, double kappa, double csw, int parity, int flags)
+{
+    QCD_REQUIRE(ctx && g && out_host && in_host && nvec >= 0, "dslash_host_batch: NULL argument or nvec < 0");
+    QCD_REQUIRE(parity == 0 || parity == 1 || parity == 2, "dslash_host_batch: parity must be 0|1|2");
+    const size_t blk = (size_t)g->geo.Vh * 24 * g->precision;
+    const size_t bytes = parity == 2 ? 2 * blk : blk;
+    QCD_REQUIRE(out_stride == 0 || out_stride >= bytes, "dslash_host_batch: out_stride smaller than a vector");
+    QCD_REQUIRE(in_stride == 0 || in_stride >= bytes, "dslash_host_batch: in_stride smaller than a vector");
+    QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= 4 * bytes + blk, "dslash_host_batch: workspace too small (need 4 fields + one parity block)");
+    if (!ctx->pipe_ready) {
+        QCD_CHECK_CUDA(cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking));
+        QCD_CHECK_CUDA(cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking));
+        QCD_CHECK_CUDA(cudaEventCreateWithFlags(&ctx->ev_start, cudaEventDisableTiming));
+        for (int b = 0; b < 2; b++) {
+            QCD_CHECK_CUDA(cudaEventCreateWithFlags(&ctx->ev_in[b], cudaEventDisableTiming));
+            QCD_CHECK_CUDA(cudaEventCreateWithFlags(&ctx->ev_comp[b], cudaEventDisableTiming));
+            QCD_CHECK_CUDA(cudaEventCreateWithFlags(&ctx->ev_out[b], cudaEventDisableTiming));
+        }
+        ctx->pipe_ready = 1;
+    }
+    char* w = (char*)ctx->ws;
+    char* d_in[2] = {w, w + bytes};
+    char* d_out[2] = {w + 2 * bytes, w + 3 * bytes};
+    char* d_tmp = w + 4 * bytes;
+    /* the copy streams start after whatever the ctx stream was doing with the workspace */
+    QCD_CHECK_CUDA(cudaEventRecord(ctx->ev_start, ctx->stream));
+    QCD_CHECK_CUDA(cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_start, 0));
+    QCD_CHECK_CUDA(cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_start, 0));
+    for (int i = 0; i < nvec; i++) {
+        const int b = i & 1;
+        /* H2D: the input buffer is free once the operator on vector i-2 has run */
+        if (i >= 2) QCD_CHECK_CUDA(cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_comp[b], 0));
+        QCD_CHECK_CUDA(cudaMemcpyAsync(d_in[b], (const char*)in_host + (size_t)i * in_stride, bytes, cudaMemcpyHostToDevice, ctx->s_h2d));
+        QCD_CHECK_CUDA(cudaEventRecord(ctx->ev_in[b], ctx->s_h2d));
+        /* operator: needs the input, and the output buffer drained by the D2H of vector i-2 */
+        QCD_CHECK_CUDA(cudaStreamWaitEvent(ctx->stream, ctx->ev_in[b], 0));
+        if (i >= 2) QCD_CHECK_CUDA(cudaStreamWaitEvent(ctx->stream, ctx->ev_out[b], 0));
+        int rc = qcd_dslash_ex(d_out[b], d_in[b], g, c, kappa, csw, parity, flags, d_tmp);
+        if (rc) return rc;
+        QCD_CHECK_CUDA(cudaEventRecord(ctx->ev_comp[b], ctx->stream));
+        /* D2H */
+        QCD_CHECK_CUDA(cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_comp[b], 0));
+        QCD_CHECK_CUDA(cudaMemcpyAsync((char*)out_host + (size_t)i * out_stride, d_out[b], bytes, cudaMemcpyDeviceToHost, ctx->s_d2h));
+        QCD_CHECK_CUDA(cudaEventRecord(ctx->ev_out[b], ctx->s_d2h));
+    }
+    QCD_CHECK_CUDA(cudaStreamSynchronize(ctx->s_d2h));
     QCD_CHECK_CUDA(cudaStreamSynchronize(ctx->stream));
     return QCD_OK;
 }

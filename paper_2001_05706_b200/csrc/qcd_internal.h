@@ -46,6 +46,10 @@ struct qcd_ctx {
     double kappa, csw, delta;
     int op_parity;
     int op_set;
+    /* qcd_dslash_host_batch: copy streams and events, created on first use */
+    cudaStream_t s_h2d, s_d2h;
+    cudaEvent_t ev_start, ev_in[2], ev_comp[2], ev_out[2];
+    int pipe_ready;
 };
 
 struct qcd_gauge {

@@ -63,6 +63,7 @@ SIGNATURES = {
     "qcd_spinor_to_half": (_i, [_vp, _vp, _vp, _dims_t, _i]),
     "qcd_spinor_from_half": (_i, [_vp, _vp, _vp, _dims_t, _i]),
     "qcd_dslash_half": (_i, [_vp, _i, _vp, _vp, _vp, _d, _d, _i, _i, _vp]),
+    "qcd_dslash_host_batch": (_i, [_vp, _vp, _vp, _i, _sz, _sz, _vp, _vp, _d, _d, _i, _i]),
     "qcd_workspace_bytes": (_sz, [_dims_t, _i]),
     "qcd_set_workspace": (_i, [_vp, _vp, _sz]),
     "qcd_axpy": (_i, [_vp, _d, _vp, _vp, _sz, _i]),
@@ -246,6 +247,15 @@ class Context:
     def dslash_host(self, out_host, in_host, gauge: "Gauge", clover, kappa: float, csw: float, parity: int, flags: int = 0):
         _check(lib().qcd_dslash_host(self.h, _ptr(out_host), _ptr(in_host), gauge.h, clover.h if clover else None,
                                      kappa, csw, parity, flags))
+
+    def dslash_host_batch(self, out_host, in_host, nvec: int, gauge: "Gauge", clover, kappa: float, csw: float,
+                          parity: int, flags: int = 0, out_stride=None, in_stride=None):
+        """nvec vectors held consecutively in (pinned) HOST tensors, pipelined H2D / operator / D2H."""
+        es = out_host.element_size()
+        ostr = out_host.numel() // max(nvec, 1) * es if out_stride is None else out_stride
+        istr = in_host.numel() // max(nvec, 1) * es if in_stride is None else in_stride
+        _check(lib().qcd_dslash_host_batch(self.h, _ptr(out_host), _ptr(in_host), nvec, ostr, istr, gauge.h,
+                                           clover.h if clover else None, kappa, csw, parity, flags))
 
     # ---- BLAS ------------------------------------------------------------------------
     def axpy(self, a, x, y):

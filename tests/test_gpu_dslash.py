@@ -184,3 +184,32 @@ def test_convert_is_layout_aware(dims):
     h = p64.numel() // 2
     one = c.convert(p64[h:], 4, dims, 1)
     assert torch.equal(one, p32[h:])
+
+
+def test_dslash_host_batch_matches_single_calls():
+    """qcd_dslash_host_batch (pipelined copies on the ctx's own copy streams) gives, vector by vector,
+    the bits qcd_dslash_host gives; covers nvec = 0, 1 and an odd count (both double buffers reused)."""
+    from paper_2001_05706_b200 import qcd
+    c = ctx()
+    dims, kappa, csw = (8, 6, 4, 10), 0.135, 1.0
+    U = inputs.gauge_field(dims, 0.5, 0)
+    g = c.gauge_load(to_dev(U, 4), dims, 4, 12, -1)
+    g64 = c.gauge_load(to_dev(U, 8), dims, 8, 18, -1)
+    cl = c.clover_build(g64, kappa, csw, 4)
+    V = int(np.prod(dims))
+    for parity, n in ((0, V // 2 * 24), (2, V * 24)):
+        c.set_workspace(None)
+        c.ensure_workspace(5 * n * 4)
+        for nvec in (0, 1, 5):
+            hin = torch.randn(max(nvec, 1) * n, dtype=torch.float32, generator=torch.Generator().manual_seed(nvec)).pin_memory()
+            hout = torch.zeros(max(nvec, 1) * n, dtype=torch.float32).pin_memory()
+            c.dslash_host_batch(hout, hin, nvec, g, cl, kappa, csw, parity, 0, out_stride=n * 4, in_stride=n * 4)
+            one = torch.zeros(n, dtype=torch.float32).pin_memory()
+            for i in range(nvec):
+                c.dslash_host(one, hin[i * n:(i + 1) * n], g, cl, kappa, csw, parity, 0)
+                assert torch.equal(one, hout[i * n:(i + 1) * n])
+            if nvec == 0:
+                assert float(hout.abs().max()) == 0.0
+    with pytest.raises(qcd.QcdError):
+        c.dslash_host_batch(hout, hin, 2, g, cl, kappa, csw, 2, 0, out_stride=16, in_stride=n * 4)
+    c.set_workspace(None)
