@@ -351,7 +351,8 @@ __device__ __forceinline__ void cheb_vector(const HopArgs<T>& A, const Links& L,
  * use of direction 0 and of z / tm / v, whose loads the compiler cannot hoist across the vector
  * loop.  Measured on B200 (48^3x96, 12 vectors, degree 100): 0 -> 1.40 s, 1 -> 1.35 s, 2 -> 1.47 s,
  * 4 -> 1.44 s, 6 -> 1.57 s, 15 -> 1.84 s; ncu on one 12-vector launch: 6.31 ms -> 6.05 ms with bit 0,
- * DRAM traffic unchanged (36.6 GB).  Requesting neighbours a vector ahead costs more than it hides. */
+ * DRAM traffic unchanged (36.6 GB).  Requesting neighbours a vector ahead costs more than it hides,
+ * and so does letting only one lane per 128-byte line issue the request (bit 0: 1.42 s). */
 template <typename T, int WHAT>
 __device__ __forceinline__ void cheb_prefetch(const HopArgs<T>& A, size_t off, size_t Vh, int cb, const Neighbours<T>& nb)
 {
