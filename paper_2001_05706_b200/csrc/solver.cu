@@ -104,7 +104,8 @@ int cg_pure(qcd_ctx* ctx, void* x, const void* b, double tol, int maxiter, qcd_s
     while (!conv && k < maxiter) {
         k++;
         RC(apply_N(o, q, p, t, tmp));
-        RC(blas_redot(ctx, p, q, o.nreal, P, d + S_PQ));
+        /* <p, N p> = <p, M^dag M p> = |M p|^2: one pass over t = M p instead of one over p and q */
+        RC(blas_norm2(ctx, t, o.nreal, P, d + S_PQ));
         RC(blas_cg_update(ctx, dev_ratio(d + cur, d + S_PQ), p, q, x, r, o.nreal, P, d + nxt, d + S_BETA, d + cur));
         RC(fetch(ctx, 0, 4));
         if (!(h[S_PQ] > 0.0)) { brk = 1; break; }
@@ -170,7 +171,10 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
         } else {
             RC(apply_N(ol, q, p, tl, l2));
         }
-        RC(blas_redot(ctx, p, q, n, 4, d + S_PQ));
+        /* <p, N p> = |M p|^2 (tl = M p); with the 16-bit operator q = M^dag store16(M p), so there
+         * the product is taken as written */
+        if (half) RC(blas_redot(ctx, p, q, n, 4, d + S_PQ));
+        else RC(blas_norm2(ctx, tl, n, 4, d + S_PQ));
         RC(blas_cg_update(ctx, dev_ratio(d + cur, d + S_PQ), p, q, x, r, n, 4, d + nxt, nullptr, nullptr));
         RC(fetch(ctx, 0, 4));
         if (!(h[S_PQ] > 0.0)) { brk = 1; break; }
@@ -198,7 +202,11 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
     }
     if (!conv) RC(blas_accumulate_hi(ctx, y, x, n, Vh));
     double r_true = 0.0;
-    RC(true_residual(oh, y, b, th, h1, h2, bnorm, &r_true));
+    /* Convergence is only ever declared by a reliable update, whose rh = b - N_hi y is the fp64
+     * residual of the returned y recomputed from scratch (O6): it is the true residual; recompute
+     * only on the other exits (maxiter, breakdown, b = 0). */
+    if (conv && nup > 0 && bnorm > 0.0) r_true = rhnorm / bnorm;
+    else RC(true_residual(oh, y, b, th, h1, h2, bnorm, &r_true));
     if (st) {
         st->iters = k; st->reliable_updates = nup; st->converged = conv; st->breakdown = brk;
         st->r_iter = bnorm > 0 ? rhnorm / bnorm : 0.0;
