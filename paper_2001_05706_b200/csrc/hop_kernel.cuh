@@ -269,6 +269,10 @@ __device__ __forceinline__ void hop_site(T (&acc)[24], const Links& L, const Src
     hop_dir<T, 3, -1, SB>(acc, L, in, cb, n.tm, n.sgn_tm);
 }
 
+#ifndef HOP_THREADS
+#define HOP_THREADS 64 /* threads per block of hop_kernel (swept on B200: 32 / 64 / 128 / 256 -> plain 12-real hop 100.7 / 100.9 /
+                          102.6 / 104.8 us); the MINBLOCKS targets below are per 128 threads */
+#endif
 #ifndef HOP_MINBLOCKS_F32
 #define HOP_MINBLOCKS_F32 4
 #endif
@@ -277,7 +281,7 @@ __device__ __forceinline__ void hop_site(T (&acc)[24], const Links& L, const Src
 #endif
 
 template <typename T, int RECON, int DAG, int MODE>
-__global__ void __launch_bounds__(128, (sizeof(T) == 4 ? HOP_MINBLOCKS_F32 : HOP_MINBLOCKS_F64)) hop_kernel(const HopArgs<T> A)
+__global__ void __launch_bounds__(HOP_THREADS, (sizeof(T) == 4 ? HOP_MINBLOCKS_F32 : HOP_MINBLOCKS_F64) * 128 / HOP_THREADS) hop_kernel(const HopArgs<T> A)
 {
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= A.geo.Vh) return;
@@ -447,7 +451,7 @@ template <typename T, int RECON> static cudaError_t hop_cheb_launch(const HopArg
 
 template <typename T, int RECON, int DAG> static cudaError_t hop_dispatch_mode(const HopArgs<T>& A, int mode, cudaStream_t st)
 {
-    const int threads = 128;
+    const int threads = HOP_THREADS;
     const int blocks = (A.geo.Vh + threads - 1) / threads;
     switch (mode) {
     case HOP_PLAIN: hop_kernel<T, RECON, DAG, HOP_PLAIN><<<blocks, threads, 0, st>>>(A); break;
