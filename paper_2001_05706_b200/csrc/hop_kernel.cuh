@@ -176,8 +176,12 @@ __device__ __forceinline__ void colour_mul(T (&w)[12], const T (&u)[18], const T
                 const int k = ADJ ? 2 * (3 * b + a) : 2 * (3 * a + b);
                 const T ur = u[k], ui = ADJ ? -u[k + 1] : u[k + 1];
                 const T hr = h[2 * (3 * j + b)], hi = h[2 * (3 * j + b) + 1];
-                re += ur * hr - ui * hi;
-                im += ur * hi + ui * hr;
+                /* one fused multiply-add per term: "re += ur*hr - ui*hi" in one statement costs three
+                 * instructions (the bracket has to be rounded before it is added) */
+                re += ur * hr;
+                re -= ui * hi;
+                im += ur * hi;
+                im += ui * hr;
             }
             w[2 * (3 * j + a)] = sign * re;
             w[2 * (3 * j + a) + 1] = sign * im;
@@ -208,8 +212,10 @@ template <typename T> __device__ __forceinline__ void clover_block_apply(T* o, c
             const int hi = i > j ? i : j, lo = i > j ? j : i;
             const int k = 6 + 2 * (5 * lo - (lo * (lo - 1)) / 2 + (hi - lo - 1));
             const T lr = c[k], li = (i > j) ? c[k + 1] : -c[k + 1];
-            re += lr * v[2 * j] - li * v[2 * j + 1];
-            im += lr * v[2 * j + 1] + li * v[2 * j];
+            re += lr * v[2 * j];
+            re -= li * v[2 * j + 1];
+            im += lr * v[2 * j + 1];
+            im += li * v[2 * j];
         }
         o[2 * i] = re;
         o[2 * i + 1] = im;

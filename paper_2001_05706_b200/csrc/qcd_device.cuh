@@ -111,10 +111,16 @@ template <typename T> __device__ __forceinline__ void reconstruct_row2(T (&u)[18
         /* (r0 x r1)_c = r0[c1] r1[c2] - r0[c2] r1[c1] */
         const T ar = u[2 * c1], ai = u[2 * c1 + 1], br = u[6 + 2 * c2], bi = u[6 + 2 * c2 + 1];
         const T cr = u[2 * c2], ci = u[2 * c2 + 1], dr = u[6 + 2 * c1], di = u[6 + 2 * c1 + 1];
-        const T re = ar * br - ai * bi - (cr * dr - ci * di);
-        const T im = ar * bi + ai * br - (cr * di + ci * dr);
+        /* one multiply and three fused multiply-adds per real (the bracketed form costs five) */
+        T re = ar * br, nim = cr * di;
+        re = re - ai * bi;
+        nim = nim + ci * dr;
+        re = re - cr * dr;
+        nim = nim - ar * bi;
+        re = re + ci * di;
+        nim = nim - ai * br;
         u[12 + 2 * c] = re;
-        u[12 + 2 * c + 1] = -im;
+        u[12 + 2 * c + 1] = nim;
     }
 }
 
