@@ -100,8 +100,10 @@ __device__ __forceinline__ void half_compute_raw2(f2 (&acc)[24], const HalfRaw& 
     const f2 d = f2_set1(1.0f / 32767.0f);
     reconstruct_row2_2(u, d);
     project2<MU, SG>(h, s);
-    /* codes -> values once, on the colour-multiplied half spinor: (norm / 32767) * (1 / 32767) */
-    const f2 scale = sign * f2_make(__fdiv_rn(ra.n, 32767.0f), __fdiv_rn(rb.n, 32767.0f)) * d;
+    /* codes -> values once, on the colour-multiplied half spinor: norm / 32767 / 32767.  Here the
+     * division is a multiplication by the rounded reciprocal (one ulp, inside the arithmetic's own
+     * rounding); the format's exact n / 32767 is kept where stored values are read back as such. */
+    const f2 scale = sign * f2_make(ra.n, rb.n) * f2_set1((1.0f / 32767.0f) * (1.0f / 32767.0f));
     colour_mul2<(DIR < 0)>(w, u, h, scale);
     reconstruct_add2<MU, SG>(acc, w);
 }
