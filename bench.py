@@ -427,6 +427,15 @@ def config_table(c, peak, config4, only4=False, cheb_degree=100):
                 "seconds_12vec_deg%d" % cheb_degree: round(sec, 4),
                 "GFLOP/s": round(HOP_FLOP * (V // 2) * nvec * 2 * cheb_degree / sec * 1e-9, 1),
                 "GB/s": round(byts / sec * 1e-9, 1), "frac": round(byts / sec * 1e-9 / peak, 4), "B/site-vector": per_sv, "clocks": clk}
+            if nb == nvec:
+                # plain multi-rhs Wilson operator (qcd_wilson_multi): in + z + out per site-vector, links once per block
+                fn = lambda: c.wilson_multi(y, v, nb, g, kappa, True)
+                ms = gpu_time_ms(fn, 10)
+                per = 288.0 + 384.0 / nb
+                res["qcd_wilson_multi, %d vectors (2 launches)" % nb] = {
+                    "ms": round(ms, 3), "GFLOP/s": round(HOP_FLOP * V * nb / (ms * 1e-3) * 1e-9, 1),
+                    "GB/s": round(per * V * nb / (ms * 1e-3) * 1e-9, 1), "frac": round(per * V * nb / (ms * 1e-3) * 1e-9 / peak, 4),
+                    "B/site-vector": per}
             del v, y
         res["note"] = "Clenshaw recurrence, gamma5 and the coefficient term fused in the hop epilogue (2 launches per degree)"
         out["config4_chebyshev_48x96_fp32_12vec_deg%d" % cheb_degree] = res

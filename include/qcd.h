@@ -229,6 +229,14 @@ int qcd_cheb_apply(qcd_ctx* ctx, void* y, const void* v, const qcd_gauge* g, dou
 int qcd_cheb_apply_multi(qcd_ctx* ctx, void* y, const void* v, int nvec, const qcd_gauge* g,
                          double kappa, const double* coeff, int degree, double scale);
 
+/* Multi-right-hand-side Wilson operator: out_j = (1 - kappa H) in_j, or
+ * gamma5 (1 - kappa H) in_j when gamma5 != 0, for nvec full-lattice vectors stored one after the
+ * other (internal layout, precision of the gauge handle: 4 | 8; no clover).  Two launches; for
+ * nvec > 1 every link is fetched from HBM once per block of 128 sites and reused from shared
+ * memory for all vectors.  out and in must not overlap. */
+int qcd_wilson_multi(qcd_ctx* ctx, void* out, const void* in, int nvec, const qcd_gauge* g,
+                     double kappa, int gamma5);
+
 /* ---- host-buffer convenience (end-to-end path: copies inside the call) -------------
  * out_host = H_{p,1-p} in_host for one-parity blocks held in HOST memory, internal
  * layout: copies in -> device scratch (ctx workspace), runs qcd_hop, copies out. */

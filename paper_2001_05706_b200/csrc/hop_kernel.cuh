@@ -34,6 +34,7 @@ template <typename T> struct HopArgs {
     int parity;
     T tb;
     T a, b, c1, c2, c3;
+    T s5; /* Chebyshev / multi-rhs epilogue: -1 applies gamma5 = diag(1,1,-1,-1), +1 does not */
 };
 
 /* ---- where a neighbour spinor comes from ---------------------------------------------- */
@@ -335,7 +336,7 @@ __device__ __forceinline__ void cheb_vector(const HopArgs<T>& A, const Links& L,
     load_planes_cs<T, 24>(zz, A.z + off, Vh, (size_t)cb);
 #pragma unroll
     for (int i = 0; i < 24; i++) {
-        const T g5 = (i < 12) ? (T)1 : (T)-1; /* gamma5 = diag(1,1,-1,-1) */
+        const T g5 = (i < 12) ? (T)1 : A.s5; /* gamma5 = diag(1,1,-1,-1) when s5 = -1 */
         acc[i] = A.c1 * g5 * (zz[i] + A.b * acc[i]);
     }
     if (A.c3 != (T)0) {
@@ -497,6 +498,7 @@ template <typename T> static HopArgs<T> make_hop_args(const qcd_gauge* g, const 
     A.parity = L.out_parity;
     A.tb = (T)g->tb;
     A.a = (T)L.a; A.b = (T)L.b; A.c1 = (T)L.c1; A.c2 = (T)L.c2; A.c3 = (T)L.c3;
+    A.s5 = (L.s5 == 0.0) ? (T)-1 : (T)L.s5;
     return A;
 }
 

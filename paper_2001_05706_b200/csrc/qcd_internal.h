@@ -104,6 +104,7 @@ struct HopLaunch {
     const void* v;        /* cheb: source vector, own parity                      */
     const void* clover;   /* A or A^-1 block of the output parity (modes 2,3)     */
     double a, b, c1, c2, c3;
+    double s5;            /* cheb: factor on spin rows 2,3 of the bracket (-1 = gamma5, +1 = none; 0 reads as -1) */
     size_t vstride;       /* cheb: reals between consecutive right-hand sides     */
     int nvec;             /* cheb: number of right-hand sides                     */
     int out_parity, dagger, mode;

@@ -454,6 +454,39 @@ int qcd_cheb_apply_multi(qcd_ctx* ctx, void* y, const void* v, int nvec, const q
     return QCD_OK;
 }
 
+/* out_j = D_W in_j = (1 - kappa H) in_j, or gamma5 D_W in_j, for nvec full-lattice vectors: two
+ * launches of the multi-rhs kernel (one per output parity), each link fetched once per block. */
+int qcd_wilson_multi(qcd_ctx* ctx, void* out, const void* in, int nvec, const qcd_gauge* g, double kappa, int gamma5)
+{
+    QCD_REQUIRE(ctx && g && out && in, "wilson_multi: NULL argument");
+    QCD_REQUIRE(g->precision == 4 || g->precision == 8, "wilson_multi: needs an fp32 or fp64 gauge handle");
+    QCD_REQUIRE(nvec >= 1, "wilson_multi: nvec must be >= 1");
+    QCD_REQUIRE((((uintptr_t)out | (uintptr_t)in) & 15u) == 0, "wilson_multi: out/in must be 16-byte aligned");
+    const int P = g->precision;
+    const size_t blk = (size_t)g->geo.Vh * 24 * P, nreal = (size_t)g->geo.V * 24;
+    const size_t batch = (size_t)nvec * 2 * blk;
+    {
+        const uintptr_t a0 = (uintptr_t)out, a1 = (uintptr_t)in;
+        QCD_REQUIRE(a0 + batch <= a1 || a1 + batch <= a0, "wilson_multi: out and in alias");
+    }
+    for (int p = 0; p < 2; p++) {
+        HopLaunch L;
+        memset(&L, 0, sizeof(L));
+        L.mode = HOP_CHEB;
+        L.in = (const char*)in + (1 - p) * blk;
+        L.z = (const char*)in + p * blk;
+        L.out = (char*)out + p * blk;
+        L.b = -kappa;
+        L.c1 = 1.0;
+        L.s5 = gamma5 ? -1.0 : 1.0;
+        L.vstride = nreal;
+        L.nvec = nvec;
+        L.out_parity = p;
+        RC(hop_launch(ctx, g, L));
+    }
+    return QCD_OK;
+}
+
 int qcd_cheb_apply(qcd_ctx* ctx, void* y, const void* v, const qcd_gauge* g, double kappa, const double* coeff, int degree, double scale)
 {
     return qcd_cheb_apply_multi(ctx, y, v, 1, g, kappa, coeff, degree, scale);

@@ -63,6 +63,7 @@ SIGNATURES = {
     "qcd_spinor_to_half": (_i, [_vp, _vp, _vp, _dims_t, _i]),
     "qcd_spinor_from_half": (_i, [_vp, _vp, _vp, _dims_t, _i]),
     "qcd_dslash_half": (_i, [_vp, _i, _vp, _vp, _vp, _d, _d, _i, _i, _vp]),
+    "qcd_wilson_multi": (_i, [_vp, _vp, _vp, _i, _vp, _d, _i]),
     "qcd_dslash_host_batch": (_i, [_vp, _vp, _vp, _i, _sz, _sz, _vp, _vp, _d, _d, _i, _i]),
     "qcd_workspace_bytes": (_sz, [_dims_t, _i]),
     "qcd_set_workspace": (_i, [_vp, _vp, _sz]),
@@ -247,6 +248,9 @@ class Context:
     def dslash_host(self, out_host, in_host, gauge: "Gauge", clover, kappa: float, csw: float, parity: int, flags: int = 0):
         _check(lib().qcd_dslash_host(self.h, _ptr(out_host), _ptr(in_host), gauge.h, clover.h if clover else None,
                                      kappa, csw, parity, flags))
+
+    def wilson_multi(self, out, inp, nvec: int, gauge: "Gauge", kappa: float, gamma5: bool = False):
+        _check(lib().qcd_wilson_multi(self.h, _ptr(out), _ptr(inp), nvec, gauge.h, kappa, int(gamma5)))
 
     def dslash_host_batch(self, out_host, in_host, nvec: int, gauge: "Gauge", clover, kappa: float, csw: float,
                           parity: int, flags: int = 0, out_stride=None, in_stride=None):

@@ -213,3 +213,28 @@ def test_dslash_host_batch_matches_single_calls():
     with pytest.raises(qcd.QcdError):
         c.dslash_host_batch(hout, hin, 2, g, cl, kappa, csw, 2, 0, out_stride=16, in_stride=n * 4)
     c.set_workspace(None)
+
+
+@pytest.mark.parametrize("precision", [4, 8])
+@pytest.mark.parametrize("dims,nvec", [((4, 4, 4, 4), 1), ((6, 4, 2, 8), 3), ((10, 6, 4, 12), 2)])
+def test_wilson_multi_matches_oracle(dims, nvec, precision):
+    """qcd_wilson_multi (links fetched once per block for all right-hand sides):
+    every vector against the oracle's D_W and gamma5 D_W."""
+    c = ctx()
+    kappa = 0.137
+    U, _ = fields(dims, 0.5, precision)
+    g = c.gauge_load(to_dev(U, precision), dims, precision, 12 if precision == 4 else 18, -1)
+    vs = [inputs.spinor_field(dims, 0, 40 + i) for i in range(nvec)]
+    if precision == 4:
+        vs = [inputs.round_to_f32(v) for v in vs]
+    batch = torch.cat([pack(c, v, dims, precision) for v in vs])
+    n = batch.numel() // nvec
+    for gamma5 in (False, True):
+        out = torch.empty_like(batch)
+        c.wilson_multi(out, batch, nvec, g, kappa, gamma5)
+        for i, v in enumerate(vs):
+            want = orc.apply_HW(v, U, dims, kappa) if gamma5 else orc.apply_M(v, U, dims, kappa)
+            assert relerr(unpack(c, out[i * n:(i + 1) * n].contiguous(), dims), want) <= TOL[precision]
+    from paper_2001_05706_b200 import qcd
+    with pytest.raises(qcd.QcdError):
+        c.wilson_multi(batch, batch, nvec, g, kappa)          # aliased
