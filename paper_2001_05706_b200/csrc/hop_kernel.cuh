@@ -489,7 +489,9 @@ template <typename T> static HopArgs<T> make_hop_args(const qcd_gauge* g, const 
     A.vstride = L.vstride;
     A.nvec = L.nvec;
     A.tblock = 1;
-    for (int tbk = 16; tbk > 1; tbk >>= 1)
+    /* t-tile of the multi-rhs traversal: swept on B200 (48^3x96, 12 vectors): 1 -> 1.45 s, 2 -> 1.41,
+     * 4 -> 1.36, 8 -> 1.36, 16 -> 1.38, 32 -> 1.42; tiling y and z as well changes nothing (1.35-1.39) */
+    for (int tbk = 8; tbk > 1; tbk >>= 1)
         if (g->geo.T % tbk == 0 && g->geo.T > tbk) { A.tblock = tbk; break; }
     A.gauge = (const T*)g->data;
     A.clover = (const T*)L.clover;
