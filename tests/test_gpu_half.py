@@ -139,3 +139,24 @@ def test_half_mixed_cg_matches_oracle(mode):
     assert abs(st.reliable_updates - st_ref["reliable_updates"]) <= 1
     assert st.r_true < 1.5 * tol
     assert relerr(got, y_ref) <= 1e-8
+
+
+def test_operator_16bit_periodic_t_boundary():
+    """t_boundary = +1 (periodic) through the 16-bit kernel: the seam sign is a lane-wise factor of
+    the packed arithmetic and must not be folded into the stored links."""
+    c = ctx()
+    dims, kappa = (6, 4, 2, 8), 0.135
+    U = inputs.gauge_field(dims, 0.5, 0)
+    g16 = c.gauge_load(to_dev(U, 8), dims, 2, 12, +1)
+    Uq = orc.q16_links(U)
+    psi = inputs.spinor_field(dims, 0, 5).astype(np.float32)
+    psi_q = orc.q16_spinor(psi)
+    p32 = c.spinor_pack(torch.from_numpy(psi).cuda(), dims)
+    ph = c.spinor_to_half(p32, dims, 2)
+    for dagger in (False, True):
+        out = torch.empty_like(p32)
+        c.dslash_half(out, 4, ph, g16, None, kappa, 0.0, 2, 1 if dagger else 0)
+        want = orc.apply_M_q16(psi_q, Uq, dims, kappa, None, None, +1, 2, dagger, False)
+        assert relerr(unpack(c, out, dims), want) <= 3e-6
+        anti = orc.apply_M_q16(psi_q, Uq, dims, kappa, None, None, -1, 2, dagger, False)
+        assert relerr(unpack(c, out, dims), anti) > 1e-3      # and it is not the antiperiodic result
