@@ -281,3 +281,41 @@ def test_half_mixed_cg_32x64_full_size(world):
     assert abs(st.reliable_updates - st_ref["reliable_updates"]) <= 1
     assert st.r_true < 1.5 * tol
     assert relerr(c.spinor_unpack(full, DIMS).cpu().numpy(), y_ref) <= 1e-8
+
+
+# ---- beyond 32-bit byte offsets ----------------------------------------------------------------
+def test_hop_64cubed_x64_offsets_beyond_4GB():
+    """64^3 x 64 (V = 16.8 M sites): the 18-real gauge field is 4.8 GB in fp32 and 9.7 GB in fp64, so
+    the (mu, parity) block offsets and plane strides no longer fit 32 bits.  Sampled sites (the last
+    time slices and the mu = 3 links live at the highest addresses) against the oracle."""
+    if _host_mem_gb() < 48:
+        pytest.skip("needs ~40 GB of host memory")
+    c = ctx()
+    dims = (64, 64, 64, 64)
+    X, Y, Z, T = dims
+    U = inputs.round_to_f32(inputs.tiled_gauge_field(dims, 0.5, 0, 8))
+    psi = inputs.round_to_f32(inputs.spinor_field(dims, 0, 0))
+    dU = torch.from_numpy(U).cuda()
+    rng = np.random.default_rng(64)
+
+    def lex64(x, y, z, t):
+        return x + X * (y + Y * (z + Z * t))
+
+    pts = [(0, 0, 0, 0), (X - 1, Y - 1, Z - 1, T - 1), (X - 1, 0, Z - 1, T - 1), (0, Y - 1, 0, T - 1), (5, 7, 63, 63), (62, 63, 63, 62)]
+    pts += [tuple(int(v) for v in rng.integers(0, [X, Y, Z, T])) for _ in range(40)]
+    S = np.array(sorted({lex64(*p) for p in pts}), dtype=np.int64)
+    want = orc.hop_sites(psi, U, dims, S, -1, False)
+    for precision, tol in ((4, 2e-6), (8, 1e-12)):
+        g = c.gauge_load(dU, dims, precision, 18, -1)
+        src = torch.from_numpy(psi)
+        pin = c.spinor_pack((src.float() if precision == 4 else src).cuda(), dims)
+        h = pin.numel() // 2
+        out = torch.zeros_like(pin)
+        c.hop(out[:h], pin[h:], g, 0, False)
+        c.hop(out[h:], pin[:h], g, 1, False)
+        got = c.spinor_unpack(out, dims).cpu().numpy().astype(np.float64).reshape(-1, 4, 3, 2)
+        assert relerr(got[S], want) <= tol
+        err = np.linalg.norm((got[S] - want).reshape(len(S), -1), axis=1) / np.linalg.norm(want.reshape(len(S), -1), axis=1)
+        assert err.max() <= 2 * tol
+        del g, pin, out, got
+        torch.cuda.empty_cache()
