@@ -250,15 +250,18 @@ def cg_mixed(b, U, dims, kappa, tol, maxiter, A=None, Ainv=None, tb=-1, mode=2, 
         Ailo = None if Ailo is None else q16_clover(Ailo)
     y = _spinor_like(dims)
     st = np.zeros(8, dtype=np.float64)
+    upd = np.zeros(256, dtype=np.int32)
     rc = lib().orc_cg_mixed(_p(y), _p(b), _p(U), None if A is None else _p(_f64(A)),
                             None if Ainv is None else _p(_f64(Ainv)), _p(Ulo),
                             None if Alo is None else _p(Alo), None if Ailo is None else _p(Ailo),
                             _dims(dims), C.c_double(kappa), C.c_int(tb), C.c_int(mode),
-                            C.c_double(tol), C.c_int(maxiter), C.c_double(delta), C.c_int(int(half)), _p(st))
+                            C.c_double(tol), C.c_int(maxiter), C.c_double(delta), C.c_int(int(half)), _p(st),
+                            _p(upd), C.c_int(len(upd)))
     if rc:
         raise MemoryError
     return y, dict(iters=int(st[0]), r_iter=st[1], r_true=st[2], converged=bool(st[3]),
-                   breakdown=bool(st[4]), reliable_updates=int(st[5]))
+                   breakdown=bool(st[4]), reliable_updates=int(st[5]),
+                   update_at=[int(k) for k in upd[:min(int(st[5]), len(upd))]])
 
 
 def cg_multishift(b, U, dims, kappa, shifts, tol, maxiter, A=None, Ainv=None, tb=-1, mode=2):

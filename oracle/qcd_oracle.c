@@ -369,12 +369,14 @@ static void apply_N_q16(fc *q, const fc *p, const orc_op_f32 *op, fc *tmp, fc *t
  *         stop iff |r_hi| <= tol|b|
  *     beta=rho'/rho; p=r+beta p (p is kept); rho=rho'
  * stats[0]=iters (fp32 N applies), [1]=last |r_hi|/|b|, [2]=true residual, [3]=converged,
- * [4]=breakdown, [5]=reliable updates.
+ * [4]=breakdown, [5]=reliable updates.  update_at (may be NULL): the iteration index k of each of
+ * the first max_updates reliable updates, reporting only (pinned against an independent
+ * dense-matrix run in tests/test_oracle_pins.py).
  */
 int orc_cg_mixed(double *y_, const double *b_, const double *Uhi, const double *Ahi,
                  const double *Ainvhi, const float *Ulo, const float *Alo, const float *Ainvlo,
                  const int *dims, double kappa, int tb, int mode, double tol, int maxiter,
-                 double delta, int half, double *stats)
+                 double delta, int half, double *stats, int *update_at, int max_updates)
 {
     const long n = (long)dims[0] * dims[1] * dims[2] * dims[3] * 12;
     orc_op_f64 ohi;
@@ -423,6 +425,7 @@ int orc_cg_mixed(double *y_, const double *b_, const double *Uhi, const double *
             rho2 = norm2_f64(rh, n);
             rhnorm = sqrt(rho2);
             rmax = rhnorm;
+            if (update_at && nup < max_updates) update_at[nup] = k;
             nup++;
             if (rhnorm <= tol * bnorm) { conv = 1; break; }
         }
@@ -608,6 +611,10 @@ int orc_apply_M_q16(float *out, const float *in, const float *U, const float *A,
  *   x_i += alpha_n (zeta_i^{n+1}/zeta_i^n) p_i ;  r -= alpha_n q ; rho_{n+1} = |r|^2
  *   stop when |r| <= tol |b|  (the smallest shift converges last: |zeta_i| <= 1)
  *   beta_n = rho_{n+1}/rho_n ;  p_i = zeta_i^{n+1} r + beta_n (zeta_i^{n+1}/zeta_i^n)^2 p_i
+ * A shifted system whose own residual |r_i| = |zeta_i^{n+1}| |r| has reached tol |b| is frozen: x_i,
+ * p_i and zeta_i are no longer updated (reading M1 in DESIGN.md).  Without this zeta_i of a large
+ * shift underflows to 0 on a long solve and the recurrence above turns 0/0 into NaN in x_i.  The
+ * shifts ascend, so the active systems are always the first `nact`.
  * x: ns consecutive fields.  stats[0]=iters, [1]=iterated |r|/|b|, [3]=converged, [4]=breakdown;
  * rtrue[i] = |b - (N + sigma_i) x_i| / |b| recomputed from scratch.
  */
@@ -634,7 +641,7 @@ int orc_cg_multishift(double *x_, const double *b_, const double *U, const doubl
     }
     const double bnorm = sqrt(norm2_f64(b, n));
     double rho = bnorm * bnorm, alpha_old = 1.0, beta_old = 0.0, rnorm = bnorm;
-    int k = 0, conv = (bnorm == 0.0), brk = 0;
+    int k = 0, conv = (bnorm == 0.0), brk = 0, nact = ns;
     while (!conv && k < maxiter) {
         k++;
         apply_N_f64(q, p, &op, tmp, t1, t2);
@@ -643,7 +650,7 @@ int orc_cg_multishift(double *x_, const double *b_, const double *U, const doubl
         const double pq = redot_f64(p, q, n);
         if (!(pq > 0.0)) { brk = 1; break; }
         const double alpha = rho / pq;
-        for (int s = 0; s < ns; s++) {
+        for (int s = 0; s < nact; s++) {
             const double sh = sigma[s] - sigma[0];
             zp[s] = z0[s] * zm[s] * alpha_old /
                     (alpha * beta_old * (zm[s] - z0[s]) + zm[s] * alpha_old * (1.0 + sh * alpha));
@@ -657,8 +664,9 @@ int orc_cg_multishift(double *x_, const double *b_, const double *U, const doubl
         const double rho2 = norm2_f64(r, n);
         rnorm = sqrt(rho2);
         if (rnorm <= tol * bnorm) { conv = 1; break; }
+        while (nact > 1 && fabs(zp[nact - 1]) * rnorm <= tol * bnorm) nact--;
         const double beta = rho2 / rho;
-        for (int s = 0; s < ns; s++) {
+        for (int s = 0; s < nact; s++) {
             const double ratio = zp[s] / z0[s], bs = beta * ratio * ratio, zs = zp[s];
             zc *ps = p + (long)s * n;
 #pragma omp parallel for schedule(static)

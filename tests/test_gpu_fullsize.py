@@ -17,6 +17,16 @@ DIMS = (32, 32, 32, 64)
 KAPPA, CSW = 0.1355, 1.0
 
 
+def assert_every_site_close(got, want, on=None, tol=4e-6):
+    """No single site may be off: |got - want|_site <= tol (|want|_site + rms |want|_site).  The rms
+    term covers sites whose result is small through cancellation among the 8 hop terms."""
+    e = np.linalg.norm((got - want).reshape(-1, 24), axis=1)
+    r = np.linalg.norm(want.reshape(-1, 24), axis=1)
+    if on is not None:
+        e, r = e[on], r[on]
+    assert (e <= tol * (r + np.sqrt(np.mean(r * r)))).all(), float((e / (r + np.sqrt(np.mean(r * r)))).max())
+
+
 def lex(x, y, z, t):
     X, Y, Z, T = DIMS
     return x + X * (y + Y * (z + Z * t))
@@ -115,6 +125,48 @@ def test_even_odd_clover_operator_sampled_sites_32x64(world, dagger):
     assert float(out[h:].abs().max()) == 0.0
 
 
+@pytest.mark.parametrize("dagger", [False, True])
+def test_even_odd_clover_operator_whole_field_32x64(world, dagger):
+    """The same call as above, compared with the oracle on EVERY even site (the oracle applies
+    Mhat at this size in well under a second once its dense clover field exists)."""
+    if _host_mem_gb() < 40:
+        pytest.skip("needs ~30 GB of host memory for the oracle's dense clover fields")
+    c, U, psi, g, g18, cl, pin = world
+    h = pin.numel() // 2
+    A = orc.clover_matrix(orc.field_strength(U, DIMS), DIMS, KAPPA * CSW)
+    Ainv = inputs.round_to_f32(orc.invert_12(A))
+    A = inputs.round_to_f32(A)
+    par = orc.parity_mask_array(DIMS)[..., None, None, None]
+    tmp = torch.empty_like(pin[:h])
+    for p in (0, 1):
+        out = torch.zeros_like(pin)
+        blk = slice(0, h) if p == 0 else slice(h, 2 * h)
+        c.dslash_ex(out[blk], pin[blk], g, cl, KAPPA, CSW, p, 1 if dagger else 0, tmp)
+        got = c.spinor_unpack(out, DIMS).cpu().numpy().astype(np.float64)
+        want = orc.apply_M(psi * (par == p), U, DIMS, KAPPA, A, Ainv, -1, p, dagger)
+        assert relerr(got, want) <= 2e-6
+        on = (par == p).ravel()
+        assert_every_site_close(got, want, on)
+        assert np.abs(got.reshape(-1, 24)[~on]).max() == 0.0        # the other parity is untouched
+        del out, got, want
+
+
+@pytest.mark.parametrize("dagger", [False, True])
+def test_hop_whole_field_32x64(world, dagger):
+    """Single-parity hop, 12- and 18-real, every site of both parities against the oracle."""
+    c, U, psi, g, g18, cl, pin = world
+    h = pin.numel() // 2
+    want = orc.hop(psi, U, DIMS, -1, dagger)
+    for gg in (g, g18):
+        out = torch.zeros_like(pin)
+        c.hop(out[:h], pin[h:], gg, 0, dagger)
+        c.hop(out[h:], pin[:h], gg, 1, dagger)
+        got = c.spinor_unpack(out, DIMS).cpu().numpy().astype(np.float64)
+        assert relerr(got, want) <= 2e-6
+        assert_every_site_close(got, want)
+        del out, got
+
+
 def test_operator_adjoint_identity_32x64(world):
     """Re<chi, Mhat psi> = Re<Mhat^dag chi, psi> on the full-size even block (any size property)."""
     c, U, psi, g, g18, cl, pin = world
@@ -137,6 +189,33 @@ def _host_mem_gb():
         return psutil.virtual_memory().available / 1e9
     except Exception:
         return 0.0
+
+
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_config1_even_odd_wilson_16x32_fp32_whole_field(recon, dagger):
+    """BASELINE.json configs[1] exactly as stated (Table 2 caption for the fp32 /
+    12-real setting): 16^3 x 32, fp32, even-odd preconditioned Wilson, eps 0.5, kappa 0.137,
+    18- and 12-real link storage; both parities, every site, against the oracle's mode 0 / 1."""
+    c = ctx()
+    dims, kappa = (16, 16, 16, 32), 0.137
+    U = inputs.round_to_f32(inputs.gauge_field(dims, 0.5, 0))
+    psi = inputs.round_to_f32(inputs.spinor_field(dims, 0, 0))
+    g = c.gauge_load(torch.from_numpy(U).float().cuda(), dims, 4, recon, -1)
+    pin = c.spinor_pack(torch.from_numpy(psi).float().cuda(), dims)
+    h = pin.numel() // 2
+    par = orc.parity_mask_array(dims)[..., None, None, None]
+    tmp = torch.empty_like(pin[:h])
+    for p in (0, 1):
+        out = torch.zeros_like(pin)
+        blk = slice(0, h) if p == 0 else slice(h, 2 * h)
+        c.dslash_ex(out[blk], pin[blk], g, None, kappa, 0.0, p, 1 if dagger else 0, tmp)
+        got = c.spinor_unpack(out, dims).cpu().numpy().astype(np.float64)
+        want = orc.apply_M(psi * (par == p), U, dims, kappa, None, None, -1, p, dagger)
+        assert relerr(got, want) <= 2e-6
+        on = (par == p).ravel()
+        assert_every_site_close(got, want, on)
+        assert np.abs(got.reshape(-1, 24)[~on]).max() == 0.0
 
 
 def test_config2_clover_cg_24x64_fp64_full_size():
