@@ -50,7 +50,8 @@ enum {
     QCD_EINVAL = -1,     /* bad argument (null / misaligned / aliased / odd dims ...) */
     QCD_EALLOC = -2,     /* small host or device scratch allocation failed           */
     QCD_ECUDA = -3,      /* CUDA runtime error (text in qcd_last_error)              */
-    QCD_EBREAKDOWN = -4  /* CG breakdown: <p,Np> <= 0 or NaN                          */
+    QCD_EBREAKDOWN = -4  /* CG breakdown: <p,Np> <= 0 or NaN; x holds the last iterate
+                            before the failing update (nothing is written by it)          */
 };
 
 enum { QCD_DAGGER = 1 };                       /* flags for qcd_dslash_ex */
@@ -66,7 +67,11 @@ typedef struct {
     int converged;         /* 1 if |r| <= tol |b| was reached                        */
     int breakdown;
     double r_iter;         /* iterated (mixed: last fp64-recomputed) residual / |b|  */
-    double r_true;         /* |b - N x| / |b| recomputed from scratch                */
+    double r_true;         /* |b - N x| / |b| in the high precision.  Pure CG: recomputed from
+                              scratch after the loop.  Mixed CG: the fp64 residual b - N_hi y of
+                              the reliable update that declared convergence (it IS the residual
+                              of the returned y, computed from scratch by that update); recomputed
+                              only on the other exits (maxiter, breakdown)                   */
     double seconds;        /* device time of the solve loop (CUDA events)            */
     double flops;          /* nominal: 1320/site hop, +504 clover; BLAS uncounted    */
     double bytes;          /* compulsory bytes moved by hop + BLAS kernels           */
@@ -206,7 +211,9 @@ int qcd_cg_solve_ex(qcd_ctx* ctx, void* x, const void* b, double tol, int maxite
  * iteration (B. Jegerlehner, hep-lat/9612014).  x: nshift consecutive fields (out), b: one
  * field, both in the precision of the (pure-precision) operator of qcd_set_operator.
  * shifts, r_true: HOST arrays; r_true (may be NULL) receives |b - (N + s_i) x_i| / |b|.
- * Stops when the base (smallest-shift) residual meets tol.  Workspace: (4 + nshift) fields. */
+ * Stops when the base (smallest-shift) residual meets tol; a shifted system whose own residual
+ * |zeta_i| |r| has met tol earlier is frozen from then on (reading M1), which also keeps
+ * zeta_i from underflowing on long solves.  Workspace: (4 + nshift) fields. */
 int qcd_cg_multishift(qcd_ctx* ctx, void* x, const void* b, const double* shifts, int nshift,
                       double tol, int maxiter, qcd_stats* stats, double* r_true);
 /* out = M in (flags & QCD_DAGGER: M^dag in) for the operator of qcd_set_operator, in

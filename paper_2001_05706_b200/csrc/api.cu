@@ -70,8 +70,12 @@ int qcd_init(int device, void* cuda_stream, qcd_ctx** out)
     if (e == cudaSuccess) e = cudaMalloc(&c->d_ticket, sizeof(unsigned int) * 64);
     if (e == cudaSuccess) e = cudaMalloc(&c->d_scalar, sizeof(double) * SC_COUNT);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_scalar, sizeof(double) * SC_COUNT);
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_ctl, sizeof(CgCtl));
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->h_status, 64, cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&c->d_status, (void*)c->h_status, 0);
     if (e == cudaSuccess) e = cudaMemset(c->d_ticket, 0, sizeof(unsigned int) * 64);
     if (e == cudaSuccess) e = cudaMemset(c->d_scalar, 0, sizeof(double) * SC_COUNT);
+    if (e == cudaSuccess) e = cudaMemset(c->d_ctl, 0, sizeof(CgCtl));
     if (e != cudaSuccess) {
         qcd_finalize(c);
         return qcd_set_error(QCD_EALLOC, "scratch allocation: %s", cudaGetErrorString(e));
@@ -83,6 +87,11 @@ int qcd_init(int device, void* cuda_stream, qcd_ctx** out)
 int qcd_finalize(qcd_ctx* c)
 {
     if (!c) return QCD_OK;
+    solver_forget_ctx(c);
+    cudaSetDevice(c->device);
+    if (c->d_ctl) cudaFree(c->d_ctl);
+    if (c->h_status) cudaFreeHost((void*)c->h_status);
+    if (c->d_hop_partial) cudaFree(c->d_hop_partial);
     if (c->d_partial) cudaFree(c->d_partial);
     if (c->d_ticket) cudaFree(c->d_ticket);
     if (c->d_scalar) cudaFree(c->d_scalar);
@@ -127,6 +136,7 @@ int qcd_gauge_load(qcd_ctx* ctx, qcd_gauge** out, const void* links, int precisi
     QCD_REQUIRE(precision != 2 || reconstruct == 12, "gauge_load: 16-bit links are stored with 12 reals");
     QCD_REQUIRE(t_boundary == 1 || t_boundary == -1, "gauge_load: t_boundary must be +1|-1");
     QCD_REQUIRE(aligned16(links) && aligned16(storage), "gauge_load: pointers must be non-NULL and 16-byte aligned");
+    QCD_ON_DEVICE(ctx);
     qcd_gauge* h = (qcd_gauge*)calloc(1, sizeof(qcd_gauge));
     if (!h) return qcd_set_error(QCD_EALLOC, "gauge handle");
     h->ctx = ctx; h->geo = g; h->precision = precision; h->reconstruct = reconstruct; h->tb = t_boundary;
@@ -156,6 +166,8 @@ int qcd_clover_build(qcd_ctx* ctx, qcd_clover** out, const qcd_gauge* g, void* s
     QCD_REQUIRE(precision == 2 || precision == 4 || precision == 8, "clover_build: precision must be 2|4|8");
     QCD_REQUIRE(g->precision != 2, "clover_build: build from an fp32 or fp64 gauge handle");
     QCD_REQUIRE(aligned16(storage), "clover_build: storage must be non-NULL and 16-byte aligned");
+    QCD_REQUIRE(g->ctx == ctx, "clover_build: the gauge handle belongs to another ctx");
+    QCD_ON_DEVICE(ctx);
     qcd_clover* c = (qcd_clover*)calloc(1, sizeof(qcd_clover));
     if (!c) return qcd_set_error(QCD_EALLOC, "clover handle");
     c->ctx = ctx; c->geo = g->geo; c->precision = precision; c->kappa = kappa; c->csw = csw;
@@ -172,6 +184,7 @@ int qcd_clover_unpack(qcd_ctx* ctx, void* dense, const qcd_clover* c, int which)
 {
     QCD_REQUIRE(ctx && c && aligned16(dense), "clover_unpack: bad argument");
     QCD_REQUIRE(which == 0 || which == 1, "clover_unpack: which must be 0|1");
+    QCD_ON_DEVICE(ctx);
     return clover_unpack(ctx, dense, c, which);
 }
 
@@ -193,6 +206,7 @@ static int pack_common(qcd_ctx* ctx, void* internal, const void* boundary, const
     QCD_REQUIRE(precision == 4 || precision == 8, "spinor pack: precision must be 4|8");
     QCD_REQUIRE(aligned16(internal) && aligned16(boundary), "spinor pack: pointers must be non-NULL, 16-byte aligned");
     QCD_REQUIRE(!overlap(internal, boundary, (size_t)g.V * 24 * precision), "spinor pack: buffers alias");
+    QCD_ON_DEVICE(ctx);
     return layout_spinor_pack(ctx, internal, boundary, g, precision, unpack);
 }
 int qcd_spinor_pack(qcd_ctx* ctx, void* internal, const void* boundary, const int dims[4], int precision)
@@ -209,6 +223,7 @@ int qcd_convert(qcd_ctx* ctx, void* dst, int pd, const void* src, int ps, const 
     QCD_REQUIRE(ctx && aligned16(dst) && aligned16(src), "convert: bad pointer");
     QCD_REQUIRE((pd == 4 || pd == 8) && (ps == 4 || ps == 8), "convert: precision must be 4|8");
     QCD_REQUIRE(nblocks == 1 || nblocks == 2, "convert: nblocks must be 1 (one parity) or 2 (full field)");
+    QCD_ON_DEVICE(ctx);
     Geom g;
     int rc = make_geom(dims, &g);
     if (rc) return rc;
@@ -242,6 +257,7 @@ int qcd_hop_xpay(void* out, const void* in, const void* z, double a, double b, c
     QCD_REQUIRE(aligned16(out) && aligned16(in), "hop: pointers must be non-NULL, 16-byte aligned");
     QCD_REQUIRE(!overlap(out, in, bytes), "hop: in and out alias");
     QCD_REQUIRE(out_parity == 0 || out_parity == 1, "hop: out_parity must be 0|1");
+    QCD_ON_DEVICE(g->ctx);
     HopLaunch L;
     memset(&L, 0, sizeof(L));
     L.out = out; L.in = in; L.out_parity = out_parity; L.dagger = dagger ? 1 : 0;
@@ -264,12 +280,20 @@ int qcd_hop(void* out, const void* in, const qcd_gauge* g, int out_parity, int d
 } /* extern "C" */
 
 /* out_p = A_pp in_p - kappa H_{p,pb} in_pb for both parities (full lattice) */
-static int apply_full(qcd_ctx* ctx, void* out, const void* in, const qcd_gauge* g, const qcd_clover* c, double kappa, int dagger)
+static int apply_full(qcd_ctx* ctx, void* out, const void* in, const qcd_gauge* g, const qcd_clover* c, double kappa, int dagger,
+                      const OpExtra* ex)
 {
     const size_t blk = (size_t)g->geo.Vh * 24 * g->precision;
     for (int p = 0; p < 2; p++) {
         HopLaunch L;
         memset(&L, 0, sizeof(L));
+        if (ex) {
+            L.halt = ex->halt;
+            if (ex->norm_out) { /* |out|^2 = even block (into norm_tmp) + odd block */
+                L.norm_out = p == 0 ? ex->norm_tmp : ex->norm_out;
+                L.norm_add = p == 0 ? nullptr : ex->norm_tmp;
+            }
+        }
         L.out = (char*)out + p * blk;
         L.in = (const char*)in + (1 - p) * blk;
         L.z = (const char*)in + p * blk;
@@ -286,16 +310,18 @@ static int apply_full(qcd_ctx* ctx, void* out, const void* in, const qcd_gauge* 
 /* even-odd Schur operator (reading O5):
  *   tmp_pb = Ainv_pb H_{pb,p} in_p ;  out_p = A_pp in_p - kappa^2 H_{p,pb} tmp_pb */
 static int apply_eo(qcd_ctx* ctx, void* out, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c, double kappa, int p,
-                    int dagger)
+                    int dagger, const OpExtra* ex)
 {
     HopLaunch L;
     memset(&L, 0, sizeof(L));
+    if (ex) L.halt = ex->halt;
     L.out = tmp; L.in = in; L.out_parity = 1 - p; L.dagger = dagger;
     if (c) { L.mode = HOP_CLOVER_OUT; L.clover = (const char*)c->data + (2 + (1 - p)) * c->block_bytes; }
     else L.mode = HOP_PLAIN;
     int rc = hop_launch(ctx, g, L);
     if (rc) return rc;
     memset(&L, 0, sizeof(L));
+    if (ex) { L.halt = ex->halt; L.norm_out = ex->norm_out; }
     L.out = out; L.in = tmp; L.z = in; L.a = 1.0; L.b = -kappa * kappa; L.out_parity = p; L.dagger = dagger;
     if (c) { L.mode = HOP_CLOVER_Z; L.clover = (const char*)c->data + p * c->block_bytes; }
     else L.mode = HOP_XPAY;
@@ -303,10 +329,10 @@ static int apply_eo(qcd_ctx* ctx, void* out, const void* in, void* tmp, const qc
 }
 
 int op_apply_M(qcd_ctx* ctx, void* out, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c, double kappa, int parity,
-               int dagger)
+               int dagger, const OpExtra* ex)
 {
-    if (parity == QCD_PARITY_FULL) return apply_full(ctx, out, in, g, c, kappa, dagger);
-    return apply_eo(ctx, out, in, tmp, g, c, kappa, parity, dagger);
+    if (parity == QCD_PARITY_FULL) return apply_full(ctx, out, in, g, c, kappa, dagger, ex);
+    return apply_eo(ctx, out, in, tmp, g, c, kappa, parity, dagger, ex);
 }
 
 extern "C" {
@@ -318,6 +344,7 @@ int qcd_dslash_ex(void* out, const void* in, const qcd_gauge* g, const qcd_clove
     QCD_REQUIRE(g->precision != 2, "dslash: 16-bit gauge handle: use qcd_dslash_half");
     qcd_ctx* ctx = g->ctx;
     QCD_REQUIRE(parity == 0 || parity == 1 || parity == 2, "dslash: parity must be 0|1|2");
+    QCD_ON_DEVICE(ctx);
     QCD_REQUIRE(aligned16(out) && aligned16(in), "dslash: pointers must be non-NULL, 16-byte aligned");
     const size_t blk = (size_t)g->geo.Vh * 24 * g->precision;
     const size_t bytes = parity == 2 ? 2 * blk : blk;
@@ -349,13 +376,14 @@ int qcd_dslash(void* out, const void* in, const qcd_gauge* g, const qcd_clover* 
 
 /* out = M in with every streamed field in 16 bits; in: 16-bit field; out: 16-bit or fp32 */
 int op_apply_M_half(qcd_ctx* ctx, void* out, int out_f32, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c,
-                    double kappa, int parity, int dagger)
+                    double kappa, int parity, int dagger, const int* halt)
 {
     const size_t hblk = (size_t)g->geo.Vh * 52, oblk = out_f32 ? (size_t)g->geo.Vh * 96 : hblk;
     HopLaunch L;
     if (parity == QCD_PARITY_FULL) {
         for (int p = 0; p < 2; p++) {
             memset(&L, 0, sizeof(L));
+            L.halt = halt;
             L.out = (char*)out + p * oblk;
             L.in = (const char*)in + (1 - p) * hblk;
             L.z = (const char*)in + p * hblk;
@@ -369,12 +397,14 @@ int op_apply_M_half(qcd_ctx* ctx, void* out, int out_f32, const void* in, void* 
     }
     const int p = parity;
     memset(&L, 0, sizeof(L));
+    L.halt = halt;
     L.out = tmp; L.in = in; L.out_parity = 1 - p; L.dagger = dagger;
     if (c) { L.mode = HOP_CLOVER_OUT; L.clover = (const char*)c->data + (2 + (1 - p)) * c->block_bytes; }
     else L.mode = HOP_PLAIN;
     int rc = hop_half_launch(ctx, g, L, 0);
     if (rc) return rc;
     memset(&L, 0, sizeof(L));
+    L.halt = halt;
     L.out = out; L.in = tmp; L.z = in; L.a = 1.0; L.b = -kappa * kappa; L.out_parity = p; L.dagger = dagger;
     if (c) { L.mode = HOP_CLOVER_Z; L.clover = (const char*)c->data + p * c->block_bytes; }
     else L.mode = HOP_XPAY;
@@ -394,6 +424,7 @@ int qcd_spinor_to_half(qcd_ctx* ctx, void* half, const void* f32, const int dims
 {
     QCD_REQUIRE(ctx && aligned16(half) && aligned16(f32), "spinor_to_half: bad pointer");
     QCD_REQUIRE(nblocks == 1 || nblocks == 2, "spinor_to_half: nblocks must be 1|2");
+    QCD_ON_DEVICE(ctx);
     Geom g;
     int rc = make_geom(dims, &g);
     if (rc) return rc;
@@ -404,6 +435,7 @@ int qcd_spinor_from_half(qcd_ctx* ctx, void* f32, const void* half, const int di
 {
     QCD_REQUIRE(ctx && aligned16(half) && aligned16(f32), "spinor_from_half: bad pointer");
     QCD_REQUIRE(nblocks == 1 || nblocks == 2, "spinor_from_half: nblocks must be 1|2");
+    QCD_ON_DEVICE(ctx);
     Geom g;
     int rc = make_geom(dims, &g);
     if (rc) return rc;
@@ -416,6 +448,7 @@ int qcd_dslash_half(void* out, int out_precision, const void* in_half, const qcd
     QCD_REQUIRE(g && g->ctx && g->precision == 2, "dslash_half: needs a 16-bit gauge handle");
     QCD_REQUIRE(out_precision == 2 || out_precision == 4, "dslash_half: out_precision must be 2|4");
     QCD_REQUIRE(parity == 0 || parity == 1 || parity == 2, "dslash_half: parity must be 0|1|2");
+    QCD_ON_DEVICE(g->ctx);
     QCD_REQUIRE(aligned16(out) && aligned16(in_half) && out != in_half, "dslash_half: bad in/out pointer");
     if (c) {
         QCD_REQUIRE(c->precision == 2 && c->geo.V == g->geo.V, "dslash_half: needs a 16-bit clover handle of the same lattice");
@@ -432,6 +465,7 @@ static int blas_args(qcd_ctx* ctx, const void* x, const void* y, size_t nreal, i
     QCD_REQUIRE(precision == 4 || precision == 8, "blas: precision must be 4|8");
     QCD_REQUIRE(nreal % 4 == 0, "blas: nreal must be a multiple of 4");
     QCD_REQUIRE(aligned16(x) && aligned16(y), "blas: pointers must be non-NULL, 16-byte aligned");
+    QCD_ON_DEVICE(ctx);
     return QCD_OK;
 }
 static int fetch_scalar(qcd_ctx* ctx, int slot, double* result)
@@ -482,7 +516,7 @@ int qcd_cg_update(qcd_ctx* ctx, double a, const void* p, const void* q, void* x,
     if (rc) return rc;
     rc = blas_args(ctx, x, r, nreal, precision);
     if (rc) return rc;
-    rc = blas_cg_update(ctx, host_scalar(a), p, q, x, r, nreal, precision, ctx->d_scalar + SC_TMP, nullptr, nullptr);
+    rc = blas_cg_update(ctx, host_scalar(a), p, q, x, r, nreal, precision, ctx->d_scalar + SC_TMP);
     if (rc || !result) return rc;
     return fetch_scalar(ctx, SC_TMP, result);
 }
@@ -491,6 +525,7 @@ int qcd_cg_update(qcd_ctx* ctx, double a, const void* p, const void* q, void* x,
 int qcd_hop_host(qcd_ctx* ctx, void* out_host, const void* in_host, const qcd_gauge* g, int out_parity, int dagger)
 {
     QCD_REQUIRE(ctx && g && out_host && in_host, "hop_host: NULL argument");
+    QCD_ON_DEVICE(ctx);
     const size_t blk = (size_t)g->geo.Vh * 24 * g->precision;
     QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= 2 * blk, "hop_host: workspace too small (qcd_set_workspace)");
     char* d_in = (char*)ctx->ws;
@@ -508,6 +543,7 @@ int qcd_dslash_host(qcd_ctx* ctx, void* out_host, const void* in_host, const qcd
 {
     QCD_REQUIRE(ctx && g && out_host && in_host, "dslash_host: NULL argument");
     QCD_REQUIRE(parity == 0 || parity == 1 || parity == 2, "dslash_host: parity must be 0|1|2");
+    QCD_ON_DEVICE(ctx);
     const size_t blk = (size_t)g->geo.Vh * 24 * g->precision;
     const size_t bytes = parity == 2 ? 2 * blk : blk;
     QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= 2 * bytes + blk, "dslash_host: workspace too small (qcd_set_workspace)");
@@ -530,6 +566,7 @@ int qcd_dslash_host_batch(qcd_ctx* ctx, void* out_host, const void* in_host, int
 {
     QCD_REQUIRE(ctx && g && out_host && in_host && nvec >= 0, "dslash_host_batch: NULL argument or nvec < 0");
     QCD_REQUIRE(parity == 0 || parity == 1 || parity == 2, "dslash_host_batch: parity must be 0|1|2");
+    QCD_ON_DEVICE(ctx);
     const size_t blk = (size_t)g->geo.Vh * 24 * g->precision;
     const size_t bytes = parity == 2 ? 2 * blk : blk;
     QCD_REQUIRE(out_stride == 0 || out_stride >= bytes, "dslash_host_batch: out_stride smaller than a vector");

@@ -21,6 +21,12 @@ __device__ __forceinline__ double eval(const DevScalar& s)
     return s.num ? s.sign * (*s.num / *s.den) : s.val;
 }
 
+/* a launch of the solver iteration does nothing while the solver's halt flag is set */
+__device__ __forceinline__ bool halted(const int* halt)
+{
+    return halt && *reinterpret_cast<const volatile int*>(halt) != 0;
+}
+
 __device__ __forceinline__ double block_sum(double v)
 {
     __shared__ double sm[BLAS_THREADS / 32];
@@ -60,9 +66,10 @@ __device__ __forceinline__ bool grid_sum(double v, double* partial, unsigned int
     return threadIdx.x == 0;
 }
 
-template <typename T> __global__ void __launch_bounds__(BLAS_THREADS) axpby_kernel(DevScalar a, const T* __restrict__ x, DevScalar b, T* __restrict__ y, size_t nvec)
+template <typename T> __global__ void __launch_bounds__(BLAS_THREADS) axpby_kernel(DevScalar a, const T* __restrict__ x, DevScalar b, T* __restrict__ y, size_t nvec, const int* halt)
 {
     typedef typename Vec<T>::type V;
+    if (halted(halt)) return;
     const T aa = (T)eval(a), bb = (T)eval(b);
     const V* xv = reinterpret_cast<const V*>(x);
     V* yv = reinterpret_cast<V*>(y);
@@ -78,9 +85,10 @@ template <typename T> __global__ void __launch_bounds__(BLAS_THREADS) axpby_kern
 }
 
 template <typename T, int TWO>
-__global__ void __launch_bounds__(BLAS_THREADS) dot_kernel(const T* __restrict__ x, const T* __restrict__ y, size_t nvec, double* partial, unsigned int* ticket, double* out)
+__global__ void __launch_bounds__(BLAS_THREADS) dot_kernel(const T* __restrict__ x, const T* __restrict__ y, size_t nvec, double* partial, unsigned int* ticket, double* out, const int* halt)
 {
     typedef typename Vec<T>::type V;
+    if (halted(halt)) return;
     const V* xv = reinterpret_cast<const V*>(x);
     const V* yv = reinterpret_cast<const V*>(y);
     double s = 0.0;
@@ -98,9 +106,23 @@ __global__ void __launch_bounds__(BLAS_THREADS) dot_kernel(const T* __restrict__
 
 template <typename T>
 __global__ void __launch_bounds__(BLAS_THREADS) cg_update_kernel(DevScalar a, const T* __restrict__ p, const T* __restrict__ q, T* __restrict__ x, T* __restrict__ r, size_t nvec, double* partial,
-                                 unsigned int* ticket, double* out, double* beta, const double* rho_old)
+                                 unsigned int* ticket, double* out, CgCtl* ctl, int* status)
 {
     typedef typename Vec<T>::type V;
+    if (ctl) {
+        if (halted(&ctl->halt)) return;
+        /* breakdown (reading O6: <p,Np> <= 0 or NaN) is detected before anything is written */
+        if (a.num && !(*a.den > 0.0)) {
+            if (blockIdx.x == 0 && threadIdx.x == 0) {
+                ctl->halt = CG_BREAKDOWN;
+                if (status) {
+                    reinterpret_cast<volatile int*>(status)[1] = CG_BREAKDOWN;
+                    __threadfence_system();
+                }
+            }
+            return;
+        }
+    }
     const T aa = (T)eval(a);
     const V* pv = reinterpret_cast<const V*>(p);
     const V* qv = reinterpret_cast<const V*>(q);
@@ -126,7 +148,28 @@ __global__ void __launch_bounds__(BLAS_THREADS) cg_update_kernel(DevScalar a, co
     double tot;
     if (grid_sum(s, partial, ticket, &tot)) {
         *out = tot;
-        if (beta) *beta = tot / *rho_old;
+        if (ctl) {
+            /* the stopping test of reading O6 / the update rule of reading O7, taken on the device */
+            const double rn = sqrt(tot);
+            const int it = ctl->iter + 1;
+            int h = CG_RUN;
+            ctl->rnorm = rn;
+            ctl->iter = it;
+            if (ctl->delta > 0.0) {
+                double rm = ctl->rmax;
+                if (rn > rm) { rm = rn; ctl->rmax = rm; }
+                if (rn < ctl->delta * rm || rn <= ctl->thresh) h = CG_UPDATE_DUE;
+            } else if (rn <= ctl->thresh) {
+                h = CG_CONVERGED;
+            }
+            if (h) ctl->halt = h;
+            if (status) {
+                volatile int* hs = reinterpret_cast<volatile int*>(status);
+                hs[1] = h;
+                __threadfence_system();
+                hs[0] = it;
+            }
+        }
     }
 }
 
@@ -158,7 +201,7 @@ __global__ void __launch_bounds__(BLAS_THREADS) accumulate_hi_kernel(double* y, 
 
 /* r_hi = b - t ; r_lo = (float) r_hi ; out = |r_hi|^2 */
 __global__ void __launch_bounds__(BLAS_THREADS) residual_hi_kernel(double* rh, float* rl, const double* b, const double* t, size_t n4, size_t Vh,
-                                   double* partial, unsigned int* ticket, double* out)
+                                   double* partial, unsigned int* ticket, double* out, CgCtl* ctl)
 {
     double s = 0.0;
     const double2* bv = reinterpret_cast<const double2*>(b);
@@ -175,7 +218,15 @@ __global__ void __launch_bounds__(BLAS_THREADS) residual_hi_kernel(double* rh, f
         lv[i] = make_float4((float)r0.x, (float)r0.y, (float)r1.x, (float)r1.y);
     }
     double tot;
-    if (grid_sum(s, partial, ticket, &tot)) *out = tot;
+    if (grid_sum(s, partial, ticket, &tot)) {
+        *out = tot;
+        if (ctl) { /* reading O7: rmax = |r_hi|; stop iff |r_hi| <= tol |b| */
+            const double rn = sqrt(tot);
+            ctl->rmax = rn;
+            ctl->rnorm = rn;
+            ctl->halt = (rn <= ctl->thresh) ? CG_CONVERGED : CG_RUN;
+        }
+    }
 }
 
 /* HI_TO_LO: lo = (float) hi ; else hi = (double) lo */
@@ -273,14 +324,14 @@ int check_launch(qcd_ctx* ctx, const char* what)
 
 } // namespace
 
-int blas_axpby(qcd_ctx* ctx, DevScalar a, const void* x, DevScalar b, void* y, size_t nreal, int prec)
+int blas_axpby(qcd_ctx* ctx, DevScalar a, const void* x, DevScalar b, void* y, size_t nreal, int prec, const int* halt)
 {
     if (prec == 4) {
         const size_t nv = nreal / 4;
-        axpby_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const float*)x, b, (float*)y, nv);
+        axpby_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const float*)x, b, (float*)y, nv, halt);
     } else {
         const size_t nv = nreal / 2;
-        axpby_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const double*)x, b, (double*)y, nv);
+        axpby_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const double*)x, b, (double*)y, nv, halt);
     }
     return check_launch(ctx, "axpby");
 }
@@ -289,37 +340,37 @@ int blas_norm2(qcd_ctx* ctx, const void* x, size_t nreal, int prec, double* d_ou
 {
     if (prec == 4) {
         const size_t nv = nreal / 4;
-        dot_kernel<float, 0><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const float*)x, (const float*)x, nv, ctx->d_partial, ctx->d_ticket, d_out);
+        dot_kernel<float, 0><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const float*)x, (const float*)x, nv, ctx->d_partial, ctx->d_ticket, d_out, nullptr);
     } else {
         const size_t nv = nreal / 2;
-        dot_kernel<double, 0><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const double*)x, (const double*)x, nv, ctx->d_partial, ctx->d_ticket, d_out);
+        dot_kernel<double, 0><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const double*)x, (const double*)x, nv, ctx->d_partial, ctx->d_ticket, d_out, nullptr);
     }
     return check_launch(ctx, "norm2");
 }
 
-int blas_redot(qcd_ctx* ctx, const void* x, const void* y, size_t nreal, int prec, double* d_out)
+int blas_redot(qcd_ctx* ctx, const void* x, const void* y, size_t nreal, int prec, double* d_out, const int* halt)
 {
     if (prec == 4) {
         const size_t nv = nreal / 4;
-        dot_kernel<float, 1><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const float*)x, (const float*)y, nv, ctx->d_partial, ctx->d_ticket, d_out);
+        dot_kernel<float, 1><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const float*)x, (const float*)y, nv, ctx->d_partial, ctx->d_ticket, d_out, halt);
     } else {
         const size_t nv = nreal / 2;
-        dot_kernel<double, 1><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const double*)x, (const double*)y, nv, ctx->d_partial, ctx->d_ticket, d_out);
+        dot_kernel<double, 1><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const double*)x, (const double*)y, nv, ctx->d_partial, ctx->d_ticket, d_out, halt);
     }
     return check_launch(ctx, "redot");
 }
 
 int blas_cg_update(qcd_ctx* ctx, DevScalar a, const void* p, const void* q, void* x, void* r, size_t nreal, int prec,
-                   double* d_out, double* d_beta, const double* d_rho_old)
+                   double* d_out, CgCtl* ctl, int* status)
 {
     if (prec == 4) {
         const size_t nv = nreal / 4;
         cg_update_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const float*)p, (const float*)q, (float*)x, (float*)r, nv,
-                                                                                   ctx->d_partial, ctx->d_ticket, d_out, d_beta, d_rho_old);
+                                                                                   ctx->d_partial, ctx->d_ticket, d_out, ctl, status);
     } else {
         const size_t nv = nreal / 2;
         cg_update_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const double*)p, (const double*)q, (double*)x, (double*)r, nv,
-                                                                                    ctx->d_partial, ctx->d_ticket, d_out, d_beta, d_rho_old);
+                                                                                    ctx->d_partial, ctx->d_ticket, d_out, ctl, status);
     }
     return check_launch(ctx, "cg_update");
 }
@@ -331,11 +382,11 @@ int blas_accumulate_hi(qcd_ctx* ctx, void* y_hi, void* x_lo, size_t nreal, size_
     return check_launch(ctx, "accumulate_hi");
 }
 
-int blas_residual_hi(qcd_ctx* ctx, void* r_hi, void* r_lo, const void* b, const void* t, size_t nreal, size_t Vh, double* d_out)
+int blas_residual_hi(qcd_ctx* ctx, void* r_hi, void* r_lo, const void* b, const void* t, size_t nreal, size_t Vh, double* d_out, CgCtl* ctl)
 {
     const size_t n4 = nreal / 4;
     residual_hi_kernel<<<grid_for(ctx, n4), BLAS_THREADS, 0, ctx->stream>>>((double*)r_hi, (float*)r_lo, (const double*)b, (const double*)t, n4, Vh,
-                                                                          ctx->d_partial, ctx->d_ticket, d_out);
+                                                                          ctx->d_partial, ctx->d_ticket, d_out, ctl);
     return check_launch(ctx, "residual_hi");
 }
 

@@ -22,6 +22,7 @@ struct HalfHopArgs {
     DevGeom geo;
     int parity;
     float tb, a, b;
+    const int* halt; /* the launch does nothing while *halt != 0 (NULL: always run) */
 };
 
 __device__ __forceinline__ void half_clover_apply(float (&o)[24], const unsigned char* clov, size_t Vh, size_t cb, const float (&v)[24])
@@ -179,6 +180,7 @@ __device__ __forceinline__ void half_store2(unsigned char* block, size_t Vh, int
 template <int DAG, int MODE, int OUT_F32>
 __global__ void __launch_bounds__(64, HOP_MINBLOCKS_HALF) hop_half_kernel(const HalfHopArgs A)
 {
+    if (A.halt && *reinterpret_cast<const volatile int*>(A.halt) != 0) return;
     /* a block of 64 threads works on 128 consecutive sites: thread t on base + t and base + 64 + t */
     const int cba = blockIdx.x * 128 + threadIdx.x;
     if (cba >= A.geo.Vh) return;
@@ -295,15 +297,20 @@ template <int TO_HALF> __global__ void half_convert_kernel(unsigned char* half, 
     }
 }
 
-/* p = a r + b p (fp32, b == 0: p not read) ; ph = store16(p) */
-__global__ void xpay_q16_kernel(float a, const float* r, float b, float* p, unsigned char* ph, size_t Vh, int nblocks)
+/* p = a r + b p (fp32; p_is_zero: p not read) ; ph = store16(p).  a, b: host values or quotients of
+ * device doubles, rounded to fp32 (reading O7: beta = (float)(rho'/rho)) */
+__global__ void xpay_q16_kernel(DevScalar as, const float* r, DevScalar bs, int p_is_zero, float* p, unsigned char* ph, size_t Vh, int nblocks,
+                                const int* halt)
 {
+    if (halt && *reinterpret_cast<const volatile int*>(halt) != 0) return;
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= Vh * (size_t)nblocks) return;
+    const float a = (float)(as.num ? as.sign * (*as.num / *as.den) : as.val);
+    const float b = p_is_zero ? 0.f : (float)(bs.num ? bs.sign * (*bs.num / *bs.den) : bs.val);
     const size_t blk = i / Vh, cb = i - blk * Vh;
     float rv[24], pv[24];
     load_planes_rw<float, 24>(rv, r + blk * 24 * Vh, Vh, cb);
-    if (b != 0.f) {
+    if (!p_is_zero) {
         load_planes_rw<float, 24>(pv, p + blk * 24 * Vh, Vh, cb);
 #pragma unroll
         for (int k = 0; k < 24; k++) pv[k] = a * rv[k] + b * pv[k];
@@ -331,6 +338,7 @@ int hop_half_launch(qcd_ctx* ctx, const qcd_gauge* g, const HopLaunch& L, int ou
     A.tb = (float)g->tb;
     A.a = (float)L.a;
     A.b = (float)L.b;
+    A.halt = L.halt;
     cudaError_t e = L.dagger ? launch_dag<1>(A, L.mode, out_f32, ctx->stream) : launch_dag<0>(A, L.mode, out_f32, ctx->stream);
     if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "half hop launch: %s", cudaGetErrorString(e));
     ctx->launches++;
@@ -349,11 +357,12 @@ int half_convert(qcd_ctx* ctx, void* half, void* f32, size_t Vh, int nblocks, in
     return QCD_OK;
 }
 
-int half_xpay_store(qcd_ctx* ctx, double a, const void* r, double b, void* p, void* ph, size_t Vh, int nblocks)
+int half_xpay_store(qcd_ctx* ctx, DevScalar a, const void* r, DevScalar b, int p_is_zero, void* p, void* ph, size_t Vh, int nblocks,
+                    const int* halt)
 {
     const size_t n = Vh * (size_t)nblocks;
     const int threads = 128, blocks = (int)((n + threads - 1) / threads);
-    xpay_q16_kernel<<<blocks, threads, 0, ctx->stream>>>((float)a, (const float*)r, (float)b, (float*)p, (unsigned char*)ph, Vh, nblocks);
+    xpay_q16_kernel<<<blocks, threads, 0, ctx->stream>>>(a, (const float*)r, b, p_is_zero, (float*)p, (unsigned char*)ph, Vh, nblocks, halt);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "half xpay: %s", cudaGetErrorString(e));
     ctx->launches++;

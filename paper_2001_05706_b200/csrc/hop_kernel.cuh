@@ -35,7 +35,58 @@ template <typename T> struct HopArgs {
     T tb;
     T a, b, c1, c2, c3;
     T s5; /* Chebyshev / multi-rhs epilogue: -1 applies gamma5 = diag(1,1,-1,-1), +1 does not */
+    /* solver hooks: gate and the norm fused into the epilogue */
+    const int* halt;        /* the launch does nothing while *halt != 0 (NULL: always run)     */
+    double* norm_out;       /* |out|^2 (+ *norm_add) in fp64, NULL = not wanted                */
+    const double* norm_add;
+    double* norm_partial;   /* one slot per block                                              */
+    unsigned int* norm_ticket;
 };
+
+/* |v|^2 of the block's sites, accumulated in fp64, one partial per block; the last block to
+ * take a ticket sums the partials in block order (deterministic for a fixed grid) and writes
+ * the result.  Called by every thread of the block (inactive threads pass active = false). */
+template <typename T, int THREADS>
+__device__ __forceinline__ void hop_fused_norm(const HopArgs<T>& A, const T (&v)[24], bool active)
+{
+    __shared__ double sm[THREADS / 32];
+    __shared__ bool last;
+    double s = 0.0;
+    if (active) {
+#pragma unroll
+        for (int i = 0; i < 24; i++) s += (double)v[i] * (double)v[i];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) sm[w] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double b = 0.0;
+#pragma unroll
+        for (int i = 0; i < THREADS / 32; i++) b += sm[i];
+        A.norm_partial[blockIdx.x] = b;
+        __threadfence();
+        const unsigned int t = atomicInc(A.norm_ticket, gridDim.x - 1); /* wraps back to 0 */
+        last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    double t = 0.0;
+    for (unsigned int i = threadIdx.x; i < gridDim.x; i += THREADS) t += ((volatile double*)A.norm_partial)[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    __syncthreads();
+    if (l == 0) sm[w] = t;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double b = A.norm_add ? *A.norm_add : 0.0;
+#pragma unroll
+        for (int i = 0; i < THREADS / 32; i++) b += sm[i];
+        *A.norm_out = b;
+    }
+}
 
 /* ---- where a neighbour spinor comes from ---------------------------------------------- */
 template <typename T> struct PlaneSpinor {
@@ -290,8 +341,14 @@ __device__ __forceinline__ void hop_site(T (&acc)[24], const Links& L, const Src
 template <typename T, int RECON, int DAG, int MODE>
 __global__ void __launch_bounds__(HOP_THREADS, (sizeof(T) == 4 ? HOP_MINBLOCKS_F32 : HOP_MINBLOCKS_F64) * 128 / HOP_THREADS) hop_kernel(const HopArgs<T> A)
 {
-    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
-    if (cb >= A.geo.Vh) return;
+    if (A.halt && *reinterpret_cast<const volatile int*>(A.halt) != 0) return;
+    int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool want_norm = (MODE == HOP_XPAY || MODE == HOP_CLOVER_Z) && A.norm_out != nullptr;
+    const bool active = cb < A.geo.Vh;
+    if (!active) {
+        if (!want_norm) return;
+        cb = A.geo.Vh - 1; /* ragged tail of a launch with a fused norm: computes a valid site, stores nothing */
+    }
     const size_t Vh = (size_t)A.geo.Vh;
     const Neighbours<T> nb(A.geo, cb, A.parity, A.tb);
     const GlobalLinks<T, RECON> L = {A.gauge, A.gblock, Vh, A.parity};
@@ -306,14 +363,16 @@ __global__ void __launch_bounds__(HOP_THREADS, (sizeof(T) == 4 ? HOP_MINBLOCKS_F
         load_planes_rw<T, 24>(zz, A.z, Vh, (size_t)cb);
 #pragma unroll
         for (int i = 0; i < 24; i++) acc[i] = A.a * zz[i] + A.b * acc[i];
-        store_planes<T, 24>(A.out, Vh, (size_t)cb, acc);
+        if (active) store_planes<T, 24>(A.out, Vh, (size_t)cb, acc);
+        if (want_norm) hop_fused_norm<T, HOP_THREADS>(A, acc, active);
     } else if (MODE == HOP_CLOVER_Z) {
         T zz[24], az[24];
         load_planes_rw<T, 24>(zz, A.z, Vh, (size_t)cb);
         clover_apply<T>(az, A.clover, Vh, (size_t)cb, zz);
 #pragma unroll
         for (int i = 0; i < 24; i++) acc[i] = A.a * az[i] + A.b * acc[i];
-        store_planes<T, 24>(A.out, Vh, (size_t)cb, acc);
+        if (active) store_planes<T, 24>(A.out, Vh, (size_t)cb, acc);
+        if (want_norm) hop_fused_norm<T, HOP_THREADS>(A, acc, active);
     } else if (MODE == HOP_CLOVER_OUT) {
         T o[24];
         clover_apply<T>(o, A.clover, Vh, (size_t)cb, acc);
@@ -446,12 +505,9 @@ template <typename T, int RECON> static cudaError_t hop_cheb_launch(const HopArg
         return cudaGetLastError();
     }
     const size_t smem = (size_t)8 * SmemLinks<T, RECON>::NCH * 128 * 16;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(hop_cheb_mrhs_kernel<T, RECON, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    /* the attribute is per device and the call is cheap: set it on every launch rather than cache it per process */
+    cudaError_t e = cudaFuncSetAttribute(hop_cheb_mrhs_kernel<T, RECON, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
     hop_cheb_mrhs_kernel<T, RECON, 1><<<blocks, threads, smem, st>>>(A);
     return cudaGetLastError();
 }
@@ -501,6 +557,11 @@ template <typename T> static HopArgs<T> make_hop_args(const qcd_gauge* g, const 
     A.tb = (T)g->tb;
     A.a = (T)L.a; A.b = (T)L.b; A.c1 = (T)L.c1; A.c2 = (T)L.c2; A.c3 = (T)L.c3;
     A.s5 = (L.s5 == 0.0) ? (T)-1 : (T)L.s5;
+    A.halt = L.halt;
+    A.norm_out = L.norm_out;
+    A.norm_add = L.norm_add;
+    A.norm_partial = g->ctx->d_hop_partial;
+    A.norm_ticket = g->ctx->d_ticket + 1; /* slot 0 belongs to blas.cu, 8 to clover.cu */
     return A;
 }
 

@@ -28,6 +28,21 @@ struct Geom {
     long long V;
 };
 
+/* Solver control block, device resident: the CG update kernel takes the
+ * stopping / reliable-update decision on the device and every kernel of the iteration returns at
+ * once while `halt` is set, so the host can enqueue iterations ahead without a synchronisation
+ * per iteration. */
+struct CgCtl {
+    double thresh;  /* tol * |b|                                                  */
+    double delta;   /* reliable-update threshold (reading O7); 0 = pure CG        */
+    double rmax;    /* max |r| since the last reliable update                     */
+    double rnorm;   /* |r| after the last executed update                         */
+    int halt;       /* 0 running, 1 converged, 2 reliable update due, 3 breakdown */
+    int iter;       /* iterations executed                                        */
+    int pad[2];
+};
+enum { CG_RUN = 0, CG_CONVERGED = 1, CG_UPDATE_DUE = 2, CG_BREAKDOWN = 3 };
+
 struct qcd_ctx {
     int device;
     cudaStream_t stream;
@@ -37,6 +52,12 @@ struct qcd_ctx {
     unsigned int* d_ticket; /* last-block tickets, one per reduction slot  */
     double* d_scalar;       /* device-resident CG scalars                  */
     double* h_scalar;       /* pinned host mirror                          */
+    CgCtl* d_ctl;           /* solver control block (device)               */
+    volatile int* h_status; /* mapped pinned host words written by the CG update kernel: [0] = iterations
+                               executed, [1] = halt code; the host polls them instead of synchronising */
+    int* d_status;          /* device address of h_status                  */
+    double* d_hop_partial;  /* per-block partials of the norm fused into the hop epilogue (grown on demand) */
+    size_t hop_partial_cap;
     int max_blocks;
     int num_sms;
     long long launches;
@@ -82,6 +103,8 @@ int qcd_set_error(int code, const char* fmt, ...);
             return qcd_set_error(QCD_ECUDA, "%s: %s (%s:%d)", #expr,                  \
                                  cudaGetErrorString(e__), __FILE__, __LINE__);        \
     } while (0)
+/* every public entry point runs on its ctx's device whatever device the caller left current */
+#define QCD_ON_DEVICE(ctx) QCD_CHECK_CUDA(cudaSetDevice((ctx)->device))
 #define QCD_REQUIRE(cond, ...)                                                        \
     do {                                                                              \
         if (!(cond)) return qcd_set_error(QCD_EINVAL, __VA_ARGS__);                   \
@@ -98,6 +121,9 @@ enum HopMode {
 
 struct HopLaunch {
     void* out;            /* one-parity block                                     */
+    const int* halt;      /* device flag: the launch does nothing while *halt != 0 (NULL = always run) */
+    double* norm_out;     /* device: receives |out|^2 (+ *norm_add), accumulated in fp64 in the epilogue (modes 1,2) */
+    const double* norm_add;
     const void* in;       /* other-parity block                                   */
     const void* z;        /* own-parity block (modes 1,2,4)                       */
     const void* tm;       /* cheb: b_{k+2}, own parity (may alias out)            */
@@ -111,19 +137,24 @@ struct HopLaunch {
 };
 
 int hop_launch(qcd_ctx* ctx, const qcd_gauge* g, const HopLaunch& L);
+void solver_forget_ctx(const qcd_ctx* ctx); /* solver.cu: qcd_finalize clears the "last ctx" of qcd_cg_solve */
 
 /* out = M in (or M^dag in): parity 2 = (A - kappa H) on the full lattice (two launches);
  * parity 0|1 = even-odd Schur operator on that parity (two launches, tmp = one parity block). */
+struct OpExtra {
+    const int* halt;   /* gate (see HopLaunch)                                                  */
+    double* norm_out;  /* device: |out|^2 of the whole result, fused into the launch(es) writing it */
+    double* norm_tmp;  /* device scratch double (full-lattice form: partial result of the first launch) */
+};
 int op_apply_M(qcd_ctx* ctx, void* out, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c,
-               double kappa, int parity, int dagger);
+               double kappa, int parity, int dagger, const OpExtra* ex = nullptr);
 
 /* ---- 16-bit storage path (hop_half.cu, api.cu) ---------------------------- */
 int hop_half_launch(qcd_ctx* ctx, const qcd_gauge* g, const HopLaunch& L, int out_f32);
 int half_convert(qcd_ctx* ctx, void* half, void* f32, size_t Vh, int nblocks, int to_half);
 /* p = a r + b p (fp32) ; ph = 16-bit copy of p */
-int half_xpay_store(qcd_ctx* ctx, double a, const void* r, double b, void* p, void* ph, size_t Vh, int nblocks);
 int op_apply_M_half(qcd_ctx* ctx, void* out, int out_f32, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c,
-                    double kappa, int parity, int dagger);
+                    double kappa, int parity, int dagger, const int* halt = nullptr);
 
 /* ---- blas.cu --------------------------------------------------------------------- */
 /* A scalar that is either a host value or the quotient of two device doubles. */
@@ -140,17 +171,25 @@ static inline DevScalar dev_ratio(const double* n, const double* d, double sign 
     return s;
 }
 
-int blas_axpby(qcd_ctx*, DevScalar a, const void* x, DevScalar b, void* y, size_t nreal, int prec);
+/* `halt` (device, may be NULL) gates a launch: it does nothing while *halt != 0 */
+int blas_axpby(qcd_ctx*, DevScalar a, const void* x, DevScalar b, void* y, size_t nreal, int prec, const int* halt = nullptr);
 int blas_norm2(qcd_ctx*, const void* x, size_t nreal, int prec, double* d_out);
-int blas_redot(qcd_ctx*, const void* x, const void* y, size_t nreal, int prec, double* d_out);
-/* x += a p; r -= a q; *d_out = |r|^2; if d_beta: *d_beta = |r|^2 / *d_rho_old */
+int blas_redot(qcd_ctx*, const void* x, const void* y, size_t nreal, int prec, double* d_out, const int* halt = nullptr);
+/* x += a p; r -= a q; *d_out = |r|^2.  With ctl: skipped while ctl->halt != 0; a breakdown (the
+ * denominator of `a` not > 0) sets halt = CG_BREAKDOWN and leaves x, r untouched; after the update
+ * the last block counts the iteration and takes the stopping / reliable-update decision
+ * (CgCtl) and mirrors (iter, halt) to the mapped host words `status`. */
 int blas_cg_update(qcd_ctx*, DevScalar a, const void* p, const void* q, void* x, void* r,
-                   size_t nreal, int prec, double* d_out, double* d_beta, const double* d_rho_old);
+                   size_t nreal, int prec, double* d_out, CgCtl* ctl = nullptr, int* status = nullptr);
 /* y(hi) += x(lo); x = 0 */
 int blas_accumulate_hi(qcd_ctx*, void* y_hi, void* x_lo, size_t nreal, size_t Vh);
-/* r_hi = b - t (fp64); r_lo = (float) r_hi; *d_out = |r_hi|^2 */
+/* r_hi = b - t (fp64); r_lo = (float) r_hi; *d_out = |r_hi|^2; with ctl: rmax = |r_hi|,
+ * halt = CG_CONVERGED if |r_hi| <= thresh else CG_RUN */
 int blas_residual_hi(qcd_ctx*, void* r_hi, void* r_lo, const void* b, const void* t, size_t nreal,
-                     size_t Vh, double* d_out);
+                     size_t Vh, double* d_out, CgCtl* ctl = nullptr);
+/* p = a r + b p (fp32) ; ph = 16-bit copy of p (hop_half.cu) */
+int half_xpay_store(qcd_ctx* ctx, DevScalar a, const void* r, DevScalar b, int p_is_zero, void* p, void* ph, size_t Vh, int nblocks,
+                    const int* halt = nullptr);
 /* internal-layout spinor blocks of Vh sites each (nreal = nblocks*24*Vh), layout-aware */
 int blas_convert(qcd_ctx*, void* dst, int pdst, const void* src, int psrc, size_t nreal, size_t Vh);
 /* multi-shift CG: ns consecutive fields of nreal reals in x and p */

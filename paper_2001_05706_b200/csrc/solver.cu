@@ -18,8 +18,10 @@ namespace {
 
 qcd_ctx* g_last_ctx = nullptr;
 
-/* device scalar slots */
-enum { S_RHO_A = 0, S_RHO_B = 1, S_PQ = 2, S_BETA = 3, S_ONE = 5, S_AUX = 6 };
+/* device scalar slots: rho before iteration k lives in slot S_RHO + ((k-1) & 1), the update of
+ * iteration k writes rho' to S_RHO + (k & 1) */
+enum { S_RHO = 0, S_PQ = 2, S_NTMP = 3, S_AUX = 6 };
+inline int rho_slot(int k) { return S_RHO + (k & 1); }
 
 struct Op {
     qcd_ctx* ctx;
@@ -40,12 +42,15 @@ Op make_op(qcd_ctx* ctx, const qcd_gauge* g, const qcd_clover* c)
     return o;
 }
 
-/* q = M^dag M p, t = M p (kept), tmp = hop temporary */
-int apply_N(const Op& o, void* q, const void* p, void* t, void* tmp)
+/* q = M^dag M p, t = M p (kept), tmp = hop temporary.  With ex: the launches are gated by
+ * ex->halt and |t|^2 = <p, M^dag M p> is accumulated in the epilogue of the launch(es) writing t
+ * (no separate pass over t). */
+int apply_N(const Op& o, void* q, const void* p, void* t, void* tmp, const OpExtra* ex = nullptr)
 {
-    int rc = op_apply_M(o.ctx, t, p, tmp, o.g, o.c, o.kappa, o.parity, 0);
+    int rc = op_apply_M(o.ctx, t, p, tmp, o.g, o.c, o.kappa, o.parity, 0, ex);
     if (rc) return rc;
-    return op_apply_M(o.ctx, q, t, tmp, o.g, o.c, o.kappa, o.parity, 1);
+    OpExtra gate = {ex ? ex->halt : nullptr, nullptr, nullptr};
+    return op_apply_M(o.ctx, q, t, tmp, o.g, o.c, o.kappa, o.parity, 1, ex ? &gate : nullptr);
 }
 
 int fetch(qcd_ctx* ctx, int slot, int n)
@@ -55,18 +60,63 @@ int fetch(qcd_ctx* ctx, int slot, int n)
     return QCD_OK;
 }
 
-int set_one(qcd_ctx* ctx)
-{
-    ctx->h_scalar[S_ONE] = 1.0;
-    QCD_CHECK_CUDA(cudaMemcpyAsync(ctx->d_scalar + S_ONE, ctx->h_scalar + S_ONE, sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
-    return QCD_OK;
-}
-
 #define RC(expr)               \
     do {                       \
         int rc__ = (expr);     \
         if (rc__) return rc__; \
     } while (0)
+
+/* ---- device-side control (CgCtl) ----------------------------------------------------------
+ * The host enqueues iterations ahead of the device; the CG update kernel decides on the device
+ * whether the iteration converged / needs a reliable update / broke down, sets ctl->halt and
+ * mirrors (iterations done, halt) into two mapped host words.  While halt is set every further
+ * kernel of the iteration returns at once, so nothing enqueued ahead changes x, r or p.  The host
+ * only polls the mapped words (no stream synchronisation per iteration). */
+int ctl_start(qcd_ctx* ctx, double thresh, double delta, double rmax)
+{
+    CgCtl* h = reinterpret_cast<CgCtl*>(ctx->h_scalar + 8); /* pinned staging (h_scalar has SC_COUNT = 16 doubles) */
+    memset(h, 0, sizeof(CgCtl));
+    h->thresh = thresh; h->delta = delta; h->rmax = rmax; h->rnorm = rmax;
+    ctx->h_status[0] = 0;
+    ctx->h_status[1] = 0;
+    QCD_CHECK_CUDA(cudaMemcpyAsync(ctx->d_ctl, h, sizeof(CgCtl), cudaMemcpyHostToDevice, ctx->stream));
+    return QCD_OK;
+}
+
+int ctl_read(qcd_ctx* ctx, CgCtl* out)
+{
+    CgCtl* h = reinterpret_cast<CgCtl*>(ctx->h_scalar + 8);
+    QCD_CHECK_CUDA(cudaMemcpyAsync(h, ctx->d_ctl, sizeof(CgCtl), cudaMemcpyDeviceToHost, ctx->stream));
+    QCD_CHECK_CUDA(cudaStreamSynchronize(ctx->stream));
+    *out = *h;
+    return QCD_OK;
+}
+
+/* block until iteration `need` has been executed or the solver halted */
+int ctl_wait(qcd_ctx* ctx, int need)
+{
+    volatile int* hs = ctx->h_status;
+    unsigned spins = 0;
+    while (hs[0] < need && hs[1] == 0) {
+        if ((++spins & 0x3ff) == 0) {
+            const cudaError_t e = cudaStreamQuery(ctx->stream);
+            if (e == cudaSuccess) return QCD_OK; /* drained: the caller reads the state */
+            if (e != cudaErrorNotReady) return qcd_set_error(QCD_ECUDA, "cg: %s", cudaGetErrorString(e));
+        }
+    }
+    return QCD_OK;
+}
+
+int run_ahead()
+{
+    /* iterations the host may be ahead of the device; each one enqueued past a halt costs a few
+     * skipped launches, each one less risks an idle device */
+    const char* e = getenv("QCD_CG_RUNAHEAD"); /* read per solve: tests sweep it */
+    int d = e ? atoi(e) : 1; /* measured on B200, 32^3x64: 0, 1, 2 within noise; 4 and 8 slower (launches skipped after every reliable update) */
+    if (d < 0) d = 0;
+    if (d > 64) d = 64;
+    return d;
+}
 
 int true_residual(const Op& o, const void* x, const void* b, void* q, void* t, void* tmp, double bnorm, double* r_true)
 {
@@ -84,6 +134,7 @@ int cg_pure(qcd_ctx* ctx, void* x, const void* b, double tol, int maxiter, qcd_s
 {
     const Op o = make_op(ctx, ctx->g_hi, ctx->c_hi);
     const int P = o.g->precision;
+    QCD_REQUIRE(P == 4 || P == 8, "cg: the operator needs an fp32 or fp64 gauge handle");
     const int nfields = o.parity == 2 ? 4 : 5;
     QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= nfields * o.bytes, "cg: workspace too small (need %zu bytes)", nfields * o.bytes);
     char* w = (char*)ctx->ws;
@@ -91,28 +142,36 @@ int cg_pure(qcd_ctx* ctx, void* x, const void* b, double tol, int maxiter, qcd_s
     double* d = ctx->d_scalar;
     double* h = ctx->h_scalar;
 
-    RC(set_one(ctx));
     RC(blas_zero(ctx, x, o.bytes));
     RC(blas_copy(ctx, r, b, o.bytes));
     RC(blas_copy(ctx, p, b, o.bytes));
-    int cur = S_RHO_A, nxt = S_RHO_B;
-    RC(blas_norm2(ctx, b, o.nreal, P, d + cur));
-    RC(fetch(ctx, cur, 1));
-    const double bnorm = sqrt(h[cur]);
+    RC(blas_norm2(ctx, b, o.nreal, P, d + rho_slot(0)));
+    RC(fetch(ctx, rho_slot(0), 1));
+    const double bnorm = sqrt(h[rho_slot(0)]);
     double rnorm = bnorm;
     int k = 0, conv = (bnorm == 0.0), brk = 0;
-    while (!conv && k < maxiter) {
-        k++;
-        RC(apply_N(o, q, p, t, tmp));
-        /* <p, N p> = <p, M^dag M p> = |M p|^2: one pass over t = M p instead of one over p and q */
-        RC(blas_norm2(ctx, t, o.nreal, P, d + S_PQ));
-        RC(blas_cg_update(ctx, dev_ratio(d + cur, d + S_PQ), p, q, x, r, o.nreal, P, d + nxt, d + S_BETA, d + cur));
-        RC(fetch(ctx, 0, 4));
-        if (!(h[S_PQ] > 0.0)) { brk = 1; break; }
-        rnorm = sqrt(h[nxt]);
-        if (rnorm <= tol * bnorm) { conv = 1; break; }
-        RC(blas_axpby(ctx, host_scalar(1.0), r, dev_ratio(d + S_BETA, d + S_ONE), p, o.nreal, P)); /* p = r + beta p */
-        const int s = cur; cur = nxt; nxt = s;
+    if (!conv && maxiter > 0) {
+        RC(ctl_start(ctx, tol * bnorm, 0.0, bnorm));
+        const int* halt = &ctx->d_ctl->halt;
+        const OpExtra ex = {halt, d + S_PQ, d + S_NTMP};
+        const int ahead = run_ahead();
+        int n = 0;
+        while (n < maxiter) {
+            n++;
+            double *rho = d + rho_slot(n - 1), *rho2 = d + rho_slot(n);
+            /* <p, N p> = |M p|^2, accumulated while t = M p is written */
+            RC(apply_N(o, q, p, t, tmp, &ex));
+            RC(blas_cg_update(ctx, dev_ratio(rho, d + S_PQ), p, q, x, r, o.nreal, P, rho2, ctx->d_ctl, ctx->d_status));
+            RC(blas_axpby(ctx, host_scalar(1.0), r, dev_ratio(rho2, rho), p, o.nreal, P, halt)); /* p = r + beta p */
+            if (n > ahead) RC(ctl_wait(ctx, n - ahead));
+            if (ctx->h_status[1]) break;
+        }
+        CgCtl c;
+        RC(ctl_read(ctx, &c));
+        conv = c.halt == CG_CONVERGED;
+        brk = c.halt == CG_BREAKDOWN;
+        k = c.iter + brk;
+        rnorm = c.rnorm;
     }
     double r_true = 0.0;
     RC(true_residual(o, x, b, q, t, tmp, bnorm, &r_true));
@@ -148,57 +207,65 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
     double* h = ctx->h_scalar;
     const size_t n = oh.nreal, Vh = (size_t)oh.g->geo.Vh;
 
-    RC(set_one(ctx));
     RC(blas_zero(ctx, y, oh.bytes));
     RC(blas_zero(ctx, x, ol.bytes));
     RC(blas_convert(ctx, r, 4, b, 8, n, Vh));
-    if (half) RC(half_xpay_store(ctx, 1.0, r, 0.0, p, ph, Vh, nblocks));
+    if (half) RC(half_xpay_store(ctx, host_scalar(1.0), r, host_scalar(0.0), 1, p, ph, Vh, nblocks));
     else RC(blas_copy(ctx, p, r, ol.bytes));
-    int cur = S_RHO_A, nxt = S_RHO_B;
     RC(blas_norm2(ctx, b, n, 8, d + S_AUX));
-    RC(blas_norm2(ctx, r, n, 4, d + cur));
+    RC(blas_norm2(ctx, r, n, 4, d + rho_slot(0)));
     RC(fetch(ctx, 0, 8));
     const double bnorm = sqrt(h[S_AUX]);
-    double rho = h[cur];
-    double rmax = sqrt(rho), rhnorm = bnorm;
+    double rhnorm = bnorm;
     int k = 0, conv = (bnorm == 0.0), brk = 0, nup = 0;
     const bool trace = getenv("QCD_TRACE") != nullptr;
-    while (!conv && k < maxiter) {
-        k++;
-        if (half) {
-            RC(op_apply_M_half(ctx, th16, 0, ph, tmp16, ol.g, ol.c, ol.kappa, ol.parity, 0));
-            RC(op_apply_M_half(ctx, q, 1, th16, tmp16, ol.g, ol.c, ol.kappa, ol.parity, 1));
-        } else {
-            RC(apply_N(ol, q, p, tl, l2));
-        }
-        /* <p, N p> = |M p|^2 (tl = M p); with the 16-bit operator q = M^dag store16(M p), so there
-         * the product is taken as written */
-        if (half) RC(blas_redot(ctx, p, q, n, 4, d + S_PQ));
-        else RC(blas_norm2(ctx, tl, n, 4, d + S_PQ));
-        RC(blas_cg_update(ctx, dev_ratio(d + cur, d + S_PQ), p, q, x, r, n, 4, d + nxt, nullptr, nullptr));
-        RC(fetch(ctx, 0, 4));
-        if (!(h[S_PQ] > 0.0)) { brk = 1; break; }
-        double rho2 = h[nxt];
-        const double rnorm = sqrt(rho2);
-        if (trace) fprintf(stderr, "mixed k=%d rho=%.6e pq=%.6e rho2=%.6e rmax=%.3e\n", k, rho, h[S_PQ], rho2, rmax);
-        if (rnorm > rmax) rmax = rnorm;
-        if (rnorm < ctx->delta * rmax || rnorm <= tol * bnorm) {
-            RC(blas_accumulate_hi(ctx, y, x, n, Vh));                 /* y += x ; x = 0          */
-            RC(apply_N(oh, th, y, h1, h2));                       /* th = N_hi y             */
-            RC(blas_residual_hi(ctx, rh, r, b, th, n, Vh, d + nxt));  /* rh = b - th ; r = (f)rh */
-            RC(fetch(ctx, nxt, 1));
-            rho2 = h[nxt];
-            rhnorm = sqrt(rho2);
-            rmax = rhnorm;
+    if (!conv && maxiter > 0) {
+        RC(ctl_start(ctx, tol * bnorm, ctx->delta, sqrt(h[rho_slot(0)])));
+        const int* halt = &ctx->d_ctl->halt;
+        const OpExtra ex = {halt, d + S_PQ, d + S_NTMP};
+        const int ahead = run_ahead();
+        int nq = 0; /* iterations enqueued (== executed whenever the device is not halted) */
+        for (;;) {
+            while (nq < maxiter) {
+                nq++;
+                double *rho = d + rho_slot(nq - 1), *rho2 = d + rho_slot(nq);
+                if (half) {
+                    /* q = M^dag store16(M store16(p)); <p, q> taken as written */
+                    RC(op_apply_M_half(ctx, th16, 0, ph, tmp16, ol.g, ol.c, ol.kappa, ol.parity, 0, halt));
+                    RC(op_apply_M_half(ctx, q, 1, th16, tmp16, ol.g, ol.c, ol.kappa, ol.parity, 1, halt));
+                    RC(blas_redot(ctx, p, q, n, 4, d + S_PQ, halt));
+                } else {
+                    RC(apply_N(ol, q, p, tl, l2, &ex)); /* <p, N p> = |M p|^2 fused into the launch writing tl = M p */
+                }
+                RC(blas_cg_update(ctx, dev_ratio(rho, d + S_PQ), p, q, x, r, n, 4, rho2, ctx->d_ctl, ctx->d_status));
+                /* p = r + beta p, beta = (float)(rho'/rho); skipped when the update halted the iteration */
+                if (half) RC(half_xpay_store(ctx, host_scalar(1.0), r, dev_ratio(rho2, rho), 0, p, ph, Vh, nblocks, halt));
+                else RC(blas_axpby(ctx, host_scalar(1.0), r, dev_ratio(rho2, rho), p, n, 4, halt));
+                if (nq > ahead) RC(ctl_wait(ctx, nq - ahead));
+                if (ctx->h_status[1]) break;
+            }
+            CgCtl c;
+            RC(ctl_read(ctx, &c));
+            k = c.iter;
+            if (c.halt == CG_RUN) break; /* maxiter */
+            if (c.halt == CG_BREAKDOWN) { brk = 1; k++; break; }
+            /* reliable update due after iteration k (reading O7) */
+            double *rho = d + rho_slot(k - 1), *rho2 = d + rho_slot(k);
+            RC(blas_accumulate_hi(ctx, y, x, n, Vh));                          /* y += x ; x = 0          */
+            RC(apply_N(oh, th, y, h1, h2));                                    /* th = N_hi y             */
+            RC(blas_residual_hi(ctx, rh, r, b, th, n, Vh, rho2, ctx->d_ctl));  /* rh = b - th ; r = (f)rh ; rho' = |rh|^2 */
+            RC(ctl_read(ctx, &c));
+            rhnorm = c.rnorm;
             nup++;
-            if (trace) fprintf(stderr, "mixed   reliable update %d: |r_hi|/|b| = %.6e\n", nup, rhnorm / bnorm);
-            if (rhnorm <= tol * bnorm) { conv = 1; break; }
+            if (trace) fprintf(stderr, "mixed   reliable update %d after iteration %d: |r_hi|/|b| = %.6e\n", nup, k, rhnorm / bnorm);
+            if (c.halt == CG_CONVERGED) { conv = 1; break; }
+            if (k >= maxiter) break;
+            ctx->h_status[1] = 0;
+            ctx->h_status[0] = k;
+            if (half) RC(half_xpay_store(ctx, host_scalar(1.0), r, dev_ratio(rho2, rho), 0, p, ph, Vh, nblocks));
+            else RC(blas_axpby(ctx, host_scalar(1.0), r, dev_ratio(rho2, rho), p, n, 4));
+            nq = k;
         }
-        const float beta = (float)(rho2 / rho);
-        if (half) RC(half_xpay_store(ctx, 1.0, r, (double)beta, p, ph, Vh, nblocks));
-        else RC(blas_axpby(ctx, host_scalar(1.0), r, host_scalar((double)beta), p, n, 4));
-        rho = rho2;
-        const int s = cur; cur = nxt; nxt = s;
     }
     if (!conv) RC(blas_accumulate_hi(ctx, y, x, n, Vh));
     double r_true = 0.0;
@@ -228,6 +295,11 @@ double hop_flops_per_apply_M(const Op& o)
 
 } // namespace
 
+void solver_forget_ctx(const qcd_ctx* ctx)
+{
+    if (g_last_ctx == ctx) g_last_ctx = nullptr;
+}
+
 extern "C" {
 
 int qcd_set_operator(qcd_ctx* ctx, const qcd_gauge* g_hi, const qcd_gauge* g_lo, const qcd_clover* c_hi, const qcd_clover* c_lo,
@@ -235,11 +307,15 @@ int qcd_set_operator(qcd_ctx* ctx, const qcd_gauge* g_hi, const qcd_gauge* g_lo,
 {
     QCD_REQUIRE(ctx && g_hi, "set_operator: NULL ctx or gauge");
     QCD_REQUIRE(parity == 0 || parity == 1 || parity == 2, "set_operator: parity must be 0|1|2");
+    QCD_REQUIRE(g_hi->ctx == ctx, "set_operator: g_hi belongs to another ctx");
+    QCD_REQUIRE(g_hi->precision == 4 || g_hi->precision == 8, "set_operator: g_hi must be an fp32 or fp64 gauge handle");
     if (c_hi) {
         QCD_REQUIRE(c_hi->precision == g_hi->precision && c_hi->geo.V == g_hi->geo.V, "set_operator: c_hi does not match g_hi");
         QCD_REQUIRE(c_hi->kappa == kappa && c_hi->csw == csw, "set_operator: kappa/csw differ from the clover's");
     }
     if (g_lo) {
+        QCD_REQUIRE(g_lo->ctx == ctx, "set_operator: g_lo belongs to another ctx");
+        QCD_REQUIRE(g_lo->precision == 2 || g_lo->precision == 4, "set_operator: g_lo must be an fp32 or 16-bit gauge handle");
         QCD_REQUIRE(g_lo->geo.V == g_hi->geo.V && g_lo->tb == g_hi->tb, "set_operator: g_lo does not match g_hi");
         QCD_REQUIRE((c_lo != nullptr) == (c_hi != nullptr), "set_operator: c_lo and c_hi must both be given or both NULL");
         if (c_lo) {
@@ -252,6 +328,18 @@ int qcd_set_operator(qcd_ctx* ctx, const qcd_gauge* g_hi, const qcd_gauge* g_lo,
     ctx->kappa = kappa; ctx->csw = csw; ctx->op_parity = parity; ctx->delta = delta;
     ctx->op_set = 1;
     g_last_ctx = ctx;
+    {
+        /* size the per-block partials of the norm fused into the hop epilogue now, not inside a solve */
+        const size_t need = ((size_t)g_hi->geo.Vh + 63) / 64;
+        if (ctx->hop_partial_cap < need) {
+            QCD_CHECK_CUDA(cudaSetDevice(ctx->device));
+            if (ctx->d_hop_partial) cudaFree(ctx->d_hop_partial);
+            ctx->d_hop_partial = nullptr;
+            ctx->hop_partial_cap = 0;
+            QCD_CHECK_CUDA(cudaMalloc(&ctx->d_hop_partial, need * sizeof(double)));
+            ctx->hop_partial_cap = need;
+        }
+    }
     return QCD_OK;
 }
 
@@ -267,6 +355,7 @@ int qcd_cg_solve_ex(qcd_ctx* ctx, void* x, const void* b, double tol, int maxite
     QCD_REQUIRE(x && b && (((uintptr_t)x | (uintptr_t)b) & 15u) == 0, "cg_solve: x/b must be non-NULL, 16-byte aligned");
     QCD_REQUIRE(x != b, "cg_solve: x and b alias");
     QCD_REQUIRE(tol > 0.0 && maxiter >= 0, "cg_solve: tol must be > 0 and maxiter >= 0");
+    QCD_ON_DEVICE(ctx);
     qcd_stats st;
     memset(&st, 0, sizeof(st));
     cudaEvent_t e0, e1;
@@ -309,6 +398,7 @@ int qcd_cg_multishift(qcd_ctx* ctx, void* x, const void* b, const double* shifts
     QCD_REQUIRE(x && b && shifts && (((uintptr_t)x | (uintptr_t)b) & 15u) == 0, "cg_multishift: bad pointer");
     QCD_REQUIRE(nshift >= 1 && nshift <= QCD_MAX_SHIFTS, "cg_multishift: 1 <= nshift <= %d", (int)QCD_MAX_SHIFTS);
     QCD_REQUIRE(tol > 0.0 && maxiter >= 0, "cg_multishift: tol must be > 0 and maxiter >= 0");
+    QCD_ON_DEVICE(ctx);
     for (int i = 0; i < nshift; i++)
         QCD_REQUIRE(shifts[i] >= 0.0 && (i == 0 || shifts[i] > shifts[i - 1]), "cg_multishift: shifts must be >= 0 and strictly ascending");
     const Op o = make_op(ctx, ctx->g_hi, ctx->c_hi);
@@ -332,13 +422,15 @@ int qcd_cg_multishift(qcd_ctx* ctx, void* x, const void* b, const double* shifts
     RC(blas_zero(ctx, x, nshift * o.bytes));
     RC(blas_copy(ctx, r, b, o.bytes));
     for (int s = 0; s < nshift; s++) RC(blas_copy(ctx, p + s * o.bytes, b, o.bytes));
-    RC(blas_norm2(ctx, b, o.nreal, P, d + S_RHO_A));
-    RC(fetch(ctx, S_RHO_A, 1));
-    const double bnorm = sqrt(h[S_RHO_A]);
-    double rho = h[S_RHO_A], alpha_old = 1.0, beta_old = 0.0, rnorm = bnorm;
+    RC(blas_norm2(ctx, b, o.nreal, P, d + S_RHO));
+    RC(fetch(ctx, S_RHO, 1));
+    const double bnorm = sqrt(h[S_RHO]);
+    double rho = h[S_RHO], alpha_old = 1.0, beta_old = 0.0, rnorm = bnorm;
     double zm[QCD_MAX_SHIFTS], z0[QCD_MAX_SHIFTS], zp[QCD_MAX_SHIFTS];
     for (int s = 0; s < nshift; s++) zm[s] = z0[s] = 1.0;
-    int k = 0, conv = (bnorm == 0.0), brk = 0;
+    /* a shifted system whose residual |zeta_s| |r| has reached tol |b| is frozen (reading M1): the
+     * shifts ascend, so the active systems are always the first nact */
+    int k = 0, conv = (bnorm == 0.0), brk = 0, nact = nshift;
     while (!conv && k < maxiter) {
         k++;
         RC(apply_N(o, q, p, t, tmp));
@@ -349,21 +441,22 @@ int qcd_cg_multishift(qcd_ctx* ctx, void* x, const void* b, const double* shifts
         if (!(pq > 0.0)) { brk = 1; break; }
         const double alpha = rho / pq;
         MultiShiftCoef cx;
-        cx.ns = nshift; cx.alpha = alpha;
-        for (int s = 0; s < nshift; s++) {
+        cx.ns = nact; cx.alpha = alpha;
+        for (int s = 0; s < nact; s++) {
             const double sh = shifts[s] - shifts[0];
             zp[s] = z0[s] * zm[s] * alpha_old / (alpha * beta_old * (zm[s] - z0[s]) + zm[s] * alpha_old * (1.0 + sh * alpha));
             cx.c[s] = alpha * zp[s] / z0[s];
         }
-        RC(blas_multishift_x(ctx, cx, x, p, q, r, o.nreal, P, d + S_RHO_B));
-        RC(fetch(ctx, S_RHO_B, 1));
-        const double rho2 = h[S_RHO_B];
+        RC(blas_multishift_x(ctx, cx, x, p, q, r, o.nreal, P, d + (S_RHO + 1)));
+        RC(fetch(ctx, (S_RHO + 1), 1));
+        const double rho2 = h[(S_RHO + 1)];
         rnorm = sqrt(rho2);
         if (rnorm <= tol * bnorm) { conv = 1; break; }
+        while (nact > 1 && fabs(zp[nact - 1]) * rnorm <= tol * bnorm) nact--;
         const double beta = rho2 / rho;
         MultiShiftCoef cz, cb;
-        cz.ns = cb.ns = nshift; cz.alpha = cb.alpha = 0.0;
-        for (int s = 0; s < nshift; s++) {
+        cz.ns = cb.ns = nact; cz.alpha = cb.alpha = 0.0;
+        for (int s = 0; s < nact; s++) {
             const double ratio = zp[s] / z0[s];
             cz.c[s] = zp[s];
             cb.c[s] = beta * ratio * ratio;
@@ -407,6 +500,9 @@ int qcd_cheb_apply_multi(qcd_ctx* ctx, void* y, const void* v, int nvec, const q
                          int degree, double scale)
 {
     QCD_REQUIRE(ctx && g && y && v && coeff, "cheb_apply: NULL argument");
+    QCD_REQUIRE(g->precision == 4 || g->precision == 8, "cheb_apply: needs an fp32 or fp64 gauge handle");
+    QCD_REQUIRE(g->ctx == ctx, "cheb_apply: the gauge handle belongs to another ctx");
+    QCD_ON_DEVICE(ctx);
     QCD_REQUIRE(degree >= 0 && scale > 0.0 && nvec >= 1, "cheb_apply: degree must be >= 0, scale > 0, nvec >= 1");
     QCD_REQUIRE((((uintptr_t)y | (uintptr_t)v) & 15u) == 0, "cheb_apply: y/v must be 16-byte aligned");
     const int P = g->precision;
@@ -461,6 +557,8 @@ int qcd_wilson_multi(qcd_ctx* ctx, void* out, const void* in, int nvec, const qc
     QCD_REQUIRE(ctx && g && out && in, "wilson_multi: NULL argument");
     QCD_REQUIRE(g->precision == 4 || g->precision == 8, "wilson_multi: needs an fp32 or fp64 gauge handle");
     QCD_REQUIRE(nvec >= 1, "wilson_multi: nvec must be >= 1");
+    QCD_REQUIRE(g->ctx == ctx, "wilson_multi: the gauge handle belongs to another ctx");
+    QCD_ON_DEVICE(ctx);
     QCD_REQUIRE((((uintptr_t)out | (uintptr_t)in) & 15u) == 0, "wilson_multi: out/in must be 16-byte aligned");
     const int P = g->precision;
     const size_t blk = (size_t)g->geo.Vh * 24 * P, nreal = (size_t)g->geo.V * 24;

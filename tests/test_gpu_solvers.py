@@ -256,3 +256,121 @@ def test_multishift_argument_errors():
         with pytest.raises(qcd.QcdError) as e:
             c.cg_multishift(x, b, bad, 1e-10, 10)
         assert e.value.code == qcd.EINVAL
+
+
+# ---- device-side control of the CG drivers ------------------------------
+@pytest.mark.parametrize("mixed", [False, True])
+def test_cg_run_ahead_does_not_change_the_iteration(mixed, monkeypatch):
+    """The host enqueues iterations ahead of the device and the kernels enqueued past the halting
+    iteration skip themselves: the result must not depend on how far ahead the host runs
+    (QCD_CG_RUNAHEAD = 0 is one poll per iteration) -- same iteration count, same bits."""
+    c = ctx()
+    dims, kappa, csw, tol = (8, 8, 8, 8), 0.1355, 1.0, 1e-10
+    U, g_hi, c_hi, A, Ainv = setup_operator(c, dims, kappa, csw, 8, 18)
+    g_lo = c.gauge_load(to_dev(U, 8), dims, 4, 12, -1) if mixed else None
+    c_lo = c.clover_build(g_hi, kappa, csw, 4) if mixed else None
+    b = inputs.spinor_field(dims, 0, 1) * (parity_mask(dims) == 0)
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    c.set_operator(g_hi, g_lo, c_hi, c_lo, kappa, csw, 0, 0.1)
+    pb = pack(c, b, dims, 8)
+    res = []
+    for ahead in ("0", "1", "2", "7"):
+        monkeypatch.setenv("QCD_CG_RUNAHEAD", ahead)
+        x = torch.zeros_like(blocks(pb)[0])
+        rc, st = c.cg_solve(x, blocks(pb)[0].clone(), tol, 5000)
+        assert rc == 0 and st.converged == 1
+        res.append((st.iters, st.reliable_updates, st.r_true, x.clone()))
+    for it, nup, rt, x in res[1:]:
+        assert (it, nup, rt) == res[0][:3]
+        assert torch.equal(x, res[0][3])
+    if mixed:
+        y_ref, st_ref = orc.cg_mixed(b, U, dims, kappa, tol, 5000, A, Ainv, -1, 0, 0.1)
+        assert abs(res[0][0] - st_ref["iters"]) <= 2 and abs(res[0][1] - st_ref["reliable_updates"]) <= 1
+
+
+@pytest.mark.parametrize("mixed", [False, True])
+def test_cg_breakdown_leaves_the_iterate_untouched(mixed):
+    """<p, N p> = NaN at the first iteration (a NaN in b): QCD_EBREAKDOWN, and the failing update
+    has written nothing -- x is still the last iterate (0), not Inf/NaN."""
+    from paper_2001_05706_b200 import qcd
+    c = ctx()
+    dims, kappa, csw = (4, 4, 4, 8), 0.135, 1.0
+    U, g_hi, c_hi, A, Ainv = setup_operator(c, dims, kappa, csw, 8, 18)
+    g_lo = c.gauge_load(to_dev(U, 8), dims, 4, 12, -1) if mixed else None
+    c_lo = c.clover_build(g_hi, kappa, csw, 4) if mixed else None
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    c.set_operator(g_hi, g_lo, c_hi, c_lo, kappa, csw, 2, 0.1)
+    pb = pack(c, inputs.spinor_field(dims, 0, 1), dims, 8)
+    pb[17] = float("nan")
+    x = torch.full_like(pb, 3.0)
+    with pytest.raises(qcd.QcdError) as e:
+        c.cg_solve(x, pb, 1e-10, 100)
+    assert e.value.code == qcd.EBREAKDOWN
+    assert float(x.abs().max()) == 0.0
+
+
+def test_mixed_cg_maxiter_matches_oracle():
+    """maxiter falls between two reliable updates: QCD_NOCONV, iters = maxiter, y = y + x."""
+    c = ctx()
+    dims, kappa, csw, tol = (4, 4, 4, 8), 0.1355, 1.0, 1e-10
+    U, g_hi, c_hi, A, Ainv = setup_operator(c, dims, kappa, csw, 8, 18)
+    g_lo = c.gauge_load(to_dev(U, 8), dims, 4, 12, -1)
+    c_lo = c.clover_build(g_hi, kappa, csw, 4)
+    b = inputs.spinor_field(dims, 0, 1)
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    c.set_operator(g_hi, g_lo, c_hi, c_lo, kappa, csw, 2, 0.1)
+    pb = pack(c, b, dims, 8)
+    for maxiter in (1, 20, 33):
+        y_ref, st_ref = orc.cg_mixed(b, U, dims, kappa, tol, maxiter, A, Ainv, -1, 2, 0.1)
+        y = torch.empty_like(pb)
+        rc, st = c.cg_solve(y, pb, tol, maxiter)
+        assert rc == 1 and st.iters == maxiter == st_ref["iters"]
+        assert st.reliable_updates == st_ref["reliable_updates"]
+        assert relerr(unpack(c, y, dims), y_ref) <= 1e-5     # fp32 inner iterate
+        assert abs(st.r_true - st_ref["r_true"]) <= 1e-3 * st_ref["r_true"]
+
+
+def test_multishift_cg_long_solve_freezes_converged_shifts():
+    """Reading M1 on the GPU: ~470 iterations at kappa = 0.2 with a shift of 10, whose zeta would
+    underflow without the freeze (NaN in x_s); every x_s finite and equal to the oracle's."""
+    c = ctx()
+    dims, kappa, tol = (4, 4, 4, 8), 0.2, 1e-10
+    shifts = [0.0, 1.0, 10.0]
+    U, g, _, _, _ = setup_operator(c, dims, kappa, 0.0, 8, 18)
+    b = inputs.spinor_field(dims, 0, 1)
+    xs_ref, st_ref = orc.cg_multishift(b, U, dims, kappa, shifts, tol, 5000)
+    pb = pack(c, b, dims, 8)
+    n = pb.numel()
+    x = torch.empty(len(shifts) * n, dtype=pb.dtype, device="cuda")
+    c.ensure_workspace((4 + len(shifts)) * n * 8)
+    c.set_operator(g, None, None, None, kappa, 0.0, 2)
+    rc, st, rts = c.cg_multishift(x, pb, shifts, tol, 5000)
+    assert rc == 0 and st.converged == 1 and st.iters > 300
+    assert abs(st.iters - st_ref["iters"]) <= 2
+    assert bool(torch.isfinite(x).all())
+    assert max(rts) < 1.5 * tol
+    for i in range(len(shifts)):
+        assert relerr(unpack(c, x[i * n:(i + 1) * n].contiguous(), dims), xs_ref[i]) <= 1e-7
+
+
+def test_solver_entry_points_reject_wrong_precision_handles():
+    """A 16-bit gauge handle where an fp32 / fp64 one is required is QCD_EINVAL, not an
+    out-of-bounds read."""
+    from paper_2001_05706_b200 import qcd
+    c = ctx()
+    dims, kappa = (4, 4, 4, 4), 0.125
+    U = inputs.gauge_field(dims, 0.5, 0)
+    g16 = c.gauge_load(to_dev(U, 8), dims, 2, 12, -1)
+    g64 = c.gauge_load(to_dev(U, 8), dims, 8, 18, -1)
+    v = torch.randn(4 ** 4 * 24, device="cuda", dtype=torch.float32)
+    y = torch.empty_like(v)
+    c.ensure_workspace(8 * v.numel() * 8)
+    with pytest.raises(qcd.QcdError) as e:
+        c.cheb_apply_multi(y, v, 1, g16, kappa, [0.5, 0.25], 2.6)
+    assert e.value.code == qcd.EINVAL
+    with pytest.raises(qcd.QcdError) as e:
+        c.set_operator(g16, None, None, None, kappa, 0.0, 2)
+    assert e.value.code == qcd.EINVAL
+    with pytest.raises(qcd.QcdError) as e:
+        c.set_operator(g64, g64, None, None, kappa, 0.0, 2)       # g_lo must be fp32 or 16-bit
+    assert e.value.code == qcd.EINVAL
