@@ -16,7 +16,8 @@ other kernel of the path (plain hop 12/18-real, fp64, the fused BLAS-1 kernels) 
 the HBM roofline, and CG / mixed-CG / Chebyshev timings.
 
 Multi-GPU: the path does not shard in this build (north_star: "Everything runs on one
-GPU"): `--gpus N` runs N independent replicas, one per rank, no data-path collective.
+GPU"): `--gpus N` runs N independent replicas, one per rank, no data-path collective
+(launched by torchrun, or by bench.py itself when no launcher set WORLD_SIZE).
 """
 from __future__ import annotations
 
@@ -48,7 +49,8 @@ def parse_args():
     ap.add_argument("--quick", action="store_true", help="skip the per-kernel / solver sections")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-solvers", action="store_true", help="kernel table only (for ncu passes)")
-    ap.add_argument("--config4", action="store_true", help="also run the 48^3x96 Chebyshev workload (configs[4])")
+    ap.add_argument("--config4", action="store_true", help="(default now) run the 48^3x96 Chebyshev workload (configs[4])")
+    ap.add_argument("--no-config4", action="store_true", help="skip the 48^3x96 Chebyshev workload (configs[4])")
     ap.add_argument("--config4-only", action="store_true", help="only the configs[4] section (for ncu passes)")
     ap.add_argument("--cheb-degree", type=int, default=100, help="Chebyshev degree timed in the configs[4] section")
     ap.add_argument("--table-scale", type=float, default=1.0, help="scale the iteration counts of the kernel table")
@@ -64,6 +66,19 @@ def measured_peaks():
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     except Exception:
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def workload_config(world):
+    """`config` of the JSON line: the same dict for our arm and for the reference arm."""
+    Vh = DIMS[0] * DIMS[1] * DIMS[2] * DIMS[3] // 2
+    return {"workload": "even-odd Wilson-clover Dslash (Mhat_ee apply = 2 fused hop launches), 32^3x64, fp32, "
+                        "12-real links, kappa 0.1355, csw 1.0, eps 0.5 (BASELINE.json configs[3] lattice, "
+                        "north_star 70% target workload)",
+            "dims": list(DIMS), "reconstruct": 12, "kappa": KAPPA, "csw": CSW, "eps": EPS,
+            "parallelism": "replicas only (x%d)" % world,
+            "l2": "inputs larger than L2 (gauge 403 MB + clover 604 MB per step) and the spinor buffers rotate over "
+                  "3 distinct sets, so no launch finds its operands left in L2 by the previous one",
+            "flop_per_step": step_flops(Vh), "gauge_recipe": "32^3x16 block of the configs[0] recipe tiled 4x in t"}
 
 
 def step_flops(Vh, clover=True):
@@ -167,19 +182,19 @@ def cpu_baseline(budget_s=15.0):
 
 
 def run_reference(args):
+    """The reference arm of this tier is the oracle as it stands, on the host cores: same metric,
+    unit and `config` as our arm, each step a bounded sample of that workload (OracleWorkload.sample).
+    Under torchrun rank 0 alone runs and prints it."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     w = OracleWorkload()
-    steps = max(1, min(args.steps, 50))
-    warm = max(1, min(args.warmup, 3))
+    steps, warm = max(1, args.steps), max(0, args.warmup)
     dt, gf = w.time_steps(steps, warm)
     line = {
         "impl": "reference", "metric": METRIC, "value": gf, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
         "warmup": warm, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "even-odd Wilson-clover Mhat apply, CPU oracle on the 16^3x32 sample of the 32^3x64 workload",
-                   "dims": list(SMALL_DIMS), "kappa": KAPPA, "csw": CSW, "eps": EPS},
+        "dtype": "f64", "data": "synthetic", "config": workload_config(max(1, args.gpus)),
         "cpu_baseline": {"value": gf, "unit": UNIT, "cores": w.cores, "kind": "oracle", "sample": w.sample},
         "e2e": {"value": gf, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -190,21 +205,31 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------
 # CUDA arm
 # ---------------------------------------------------------------------------------------
+NSETS = 3   # distinct operand sets the timed loops rotate over (a 101 MB spinor block fits
+            # the 126 MB L2, so back-to-back launches on ONE set find part of their input still cached)
+
+
 def gpu_time_ms(fn, iters, warm=3):
-    """Average device time of fn() in ms: CUDA events on the launching stream (the ctx is
-    bound to torch's current stream), after warm-up, synchronised on both sides."""
+    """Average device time of fn(i) in ms: CUDA events on the launching stream (the ctx is
+    bound to torch's current stream), after warm-up, synchronised on both sides.  fn gets the
+    iteration number and picks operand set i % NSETS."""
     import torch
     iters = max(1, int(iters * TABLE_SCALE))
-    for _ in range(warm if TABLE_SCALE >= 1.0 else 1):
-        fn()
+    for i in range(warm if TABLE_SCALE >= 1.0 else 1):
+        fn(i)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    for _ in range(iters):
-        fn()
+    for i in range(iters):
+        fn(i)
     e1.record()
     e1.synchronize()
     return e0.elapsed_time(e1) / iters
+
+
+def sets_of(t, n=NSETS):
+    """n distinct copies of a device tensor"""
+    return [t.clone() for _ in range(n)]
 
 
 def build_workload(c, dims, want_hi):
@@ -260,35 +285,40 @@ def kernel_table(c, w, peak):
                      "GFLOP/s": round(flop_per_site * Vh / (ms * 1e-3) * 1e-9, 1), "B/site": bytes_per_site}
 
     h = Vh * 24
-    a32, b32 = w["psi32"][:h], torch.empty_like(w["psi32"][:h])
-    z32 = w["psi32"][h:]
-    row("hop_fp32_12", gpu_time_ms(lambda: c.hop(b32, z32, w["g32"], 0), 50), 576, 1320)
-    row("hop_fp32_18", gpu_time_ms(lambda: c.hop(b32, z32, w["g32_18"], 0), 50), 768, 1320)
-    row("hop_xpay_fp32_12", gpu_time_ms(lambda: c.hop_xpay(b32, z32, a32, 1.0, -KAPPA, w["g32"], 0), 50), 672, 1320)
-    a64, b64 = w["psi64"][:h], torch.empty_like(w["psi64"][:h])
-    z64 = w["psi64"][h:]
-    row("hop_fp64_18", gpu_time_ms(lambda: c.hop(b64, z64, w["g64"], 0), 20), 1536, 1320)
-    tmp64 = torch.empty_like(b64)
-    ms = gpu_time_ms(lambda: c.dslash_ex(b64, a64, w["g64"], w["c64"], KAPPA, CSW, 0, 0, tmp64), 20)
+    R = range(NSETS)
+    a32, z32 = sets_of(w["psi32"][:h]), sets_of(w["psi32"][h:])
+    b32 = [torch.empty_like(a32[0]) for _ in R]
+    row("hop_fp32_12", gpu_time_ms(lambda i: c.hop(b32[i % NSETS], z32[i % NSETS], w["g32"], 0), 60), 576, 1320)
+    row("hop_fp32_18", gpu_time_ms(lambda i: c.hop(b32[i % NSETS], z32[i % NSETS], w["g32_18"], 0), 60), 768, 1320)
+    row("hop_xpay_fp32_12", gpu_time_ms(lambda i: c.hop_xpay(b32[i % NSETS], z32[i % NSETS], a32[i % NSETS], 1.0, -KAPPA, w["g32"], 0), 60), 672, 1320)
+    a64, z64 = sets_of(w["psi64"][:h]), sets_of(w["psi64"][h:])
+    b64 = [torch.empty_like(a64[0]) for _ in R]
+    tmp64 = [torch.empty_like(a64[0]) for _ in R]
+    row("hop_fp64_18", gpu_time_ms(lambda i: c.hop(b64[i % NSETS], z64[i % NSETS], w["g64"], 0), 21), 1536, 1320)
+    ms = gpu_time_ms(lambda i: c.dslash_ex(b64[i % NSETS], a64[i % NSETS], w["g64"], w["c64"], KAPPA, CSW, 0, 0, tmp64[i % NSETS]), 21)
     row("Mhat_clover_fp64_18 (2 launches)", ms, 2 * 1536 + 2 * 576 + 192, 2 * 1320 + 2 * 504)
+    del a64, z64, b64, tmp64
     # 16-bit storage (reading H1): 52 B spinor site, 24 B link, 148 B clover site
-    ph = c.spinor_to_half(w["psi32"], dims, 2)
     hb = Vh * 52
-    o16, t16 = c.empty(hb), c.empty(hb)
-    ms = gpu_time_ms(lambda: c.dslash_half(o16, 2, ph[:hb], w["g16"], None, KAPPA, 0.0, 0, 0, t16), 50)
+    ph = sets_of(c.spinor_to_half(w["psi32"], dims, 2)[:hb])
+    o16, t16 = [c.empty(hb) for _ in R], [c.empty(hb) for _ in R]
+    ms = gpu_time_ms(lambda i: c.dslash_half(o16[i % NSETS], 2, ph[i % NSETS], w["g16"], None, KAPPA, 0.0, 0, 0, t16[i % NSETS]), 60)
     row("Mhat_wilson_q16_12 (2 launches: hop, hop+xpay)", ms, 2 * (52 + 192 + 52) + 52, 2 * 1320)
-    ms = gpu_time_ms(lambda: c.dslash_half(o16, 2, ph[:hb], w["g16"], w["c16"], KAPPA, CSW, 0, 0, t16), 50)
+    ms = gpu_time_ms(lambda i: c.dslash_half(o16[i % NSETS], 2, ph[i % NSETS], w["g16"], w["c16"], KAPPA, CSW, 0, 0, t16[i % NSETS]), 60)
     row("Mhat_clover_q16_12 (2 launches)", ms, 2 * (52 + 192 + 148 + 52) + 52, 2 * 1320 + 2 * 504)
-    # fused BLAS-1, one-parity fp32 vectors (100 MB each; 4 distinct arrays > L2)
-    x, y, p, q = (torch.randn(h, device="cuda", dtype=torch.float32) for _ in range(4))
-    row("axpy_fp32", gpu_time_ms(lambda: c.axpy(1e-3, x, y), 50), 288, 48)
-    row("xpay_fp32", gpu_time_ms(lambda: c.xpay(x, 0.5, y), 50), 288, 48)
-    row("norm2_fp32", gpu_time_ms(lambda: c.norm2(x, fetch=False), 50), 96, 48)
-    row("redot_fp32", gpu_time_ms(lambda: c.redot(x, y, fetch=False), 50), 192, 96)
-    row("cg_update_fp32", gpu_time_ms(lambda: c.cg_update(1e-6, p, q, x, y, fetch=False), 50), 576, 144)
-    x, y, p, q = (t.double() for t in (x, y, p, q))
-    row("cg_update_fp64", gpu_time_ms(lambda: c.cg_update(1e-6, p, q, x, y, fetch=False), 20), 1152, 144)
-    row("redot_fp64", gpu_time_ms(lambda: c.redot(x, y, fetch=False), 20), 384, 96)
+    del ph, o16, t16
+    # fused BLAS-1, one-parity vectors (100 MB each in fp32); NSETS sets of 4 distinct arrays
+    X, Y, P, Q = ([torch.randn(h, device="cuda", dtype=torch.float32) for _ in R] for _ in range(4))
+    row("axpy_fp32", gpu_time_ms(lambda i: c.axpy(1e-3, X[i % NSETS], Y[i % NSETS]), 60), 288, 48)
+    row("xpay_fp32", gpu_time_ms(lambda i: c.xpay(X[i % NSETS], 0.5, Y[i % NSETS]), 60), 288, 48)
+    row("norm2_fp32", gpu_time_ms(lambda i: c.norm2(X[i % NSETS], fetch=False), 60), 96, 48)
+    row("redot_fp32", gpu_time_ms(lambda i: c.redot(X[i % NSETS], Y[i % NSETS], fetch=False), 60), 192, 96)
+    row("cg_update_fp32", gpu_time_ms(lambda i: c.cg_update(1e-6, P[i % NSETS], Q[i % NSETS], X[i % NSETS], Y[i % NSETS], fetch=False), 60), 576, 144)
+    X, Y, P, Q = ([t.double() for t in v] for v in (X, Y, P, Q))
+    row("cg_update_fp64", gpu_time_ms(lambda i: c.cg_update(1e-6, P[i % NSETS], Q[i % NSETS], X[i % NSETS], Y[i % NSETS], fetch=False), 21), 1152, 144)
+    row("redot_fp64", gpu_time_ms(lambda i: c.redot(X[i % NSETS], Y[i % NSETS], fetch=False), 21), 384, 96)
+    row("norm2_fp64", gpu_time_ms(lambda i: c.norm2(X[i % NSETS], fetch=False), 21), 192, 48)
+    row("axpy_fp64", gpu_time_ms(lambda i: c.axpy(1e-3, X[i % NSETS], Y[i % NSETS]), 21), 576, 48)
     return out
 
 
@@ -345,7 +375,7 @@ def config_table(c, peak, config4, only4=False, cheb_degree=100):
         cgx = qcd.Context(torch.cuda.current_device(), stream=gs)   # a ctx on a capturable side stream
         for rec in (18, 12):
             g = c.gauge_load(dU, dims, 4, rec, -1)
-            fn = lambda: c.dslash_ex(dst, src, g, None, kappa, 0.0, 0, 0, tmp)
+            fn = lambda i=0: c.dslash_ex(dst, src, g, None, kappa, 0.0, 0, 0, tmp)
             loop_ms = gpu_time_ms(fn, 100)
             # the same 100-apply loop captured once in a CUDA graph and replayed (SURVEY 8(d) caveat i)
             gs.wait_stream(torch.cuda.current_stream())
@@ -429,8 +459,7 @@ def config_table(c, peak, config4, only4=False, cheb_degree=100):
                 "GB/s": round(byts / sec * 1e-9, 1), "frac": round(byts / sec * 1e-9 / peak, 4), "B/site-vector": per_sv, "clocks": clk}
             if nb == nvec:
                 # plain multi-rhs Wilson operator (qcd_wilson_multi): in + z + out per site-vector, links once per block
-                fn = lambda: c.wilson_multi(y, v, nb, g, kappa, True)
-                ms = gpu_time_ms(fn, 10)
+                ms = gpu_time_ms(lambda i: c.wilson_multi(y, v, nb, g, kappa, True), 10)
                 per = 288.0 + 384.0 / nb
                 res["qcd_wilson_multi, %d vectors (2 launches)" % nb] = {
                     "ms": round(ms, 3), "GFLOP/s": round(HOP_FLOP * V * nb / (ms * 1e-3) * 1e-9, 1),
@@ -484,16 +513,19 @@ def run_ours(args):
     dims = DIMS
     Vh = dims[0] * dims[1] * dims[2] * dims[3] // 2
     h = Vh * 24
-    src, dst = w["psi32"][:h], torch.empty_like(w["psi32"][:h])
-    tmp = torch.empty_like(dst)
+    srcs = sets_of(w["psi32"][:h])
+    dsts = [torch.empty_like(srcs[0]) for _ in range(NSETS)]
+    tmps = [torch.empty_like(srcs[0]) for _ in range(NSETS)]
+    src = srcs[0]
     g, cl = w["g32"], w["c32"]
 
-    def step():
-        c.dslash_ex(dst, src, g, cl, KAPPA, CSW, 0, 0, tmp)
+    def step(i=0):
+        k = i % NSETS
+        c.dslash_ex(dsts[k], srcs[k], g, cl, KAPPA, CSW, 0, 0, tmps[k])
 
     # ---- timed region: W warm-up steps, then exactly K steps between barrier + synchronize
-    for _ in range(max(args.warmup, 3)):
-        step()
+    for i in range(max(args.warmup, 3)):
+        step(i)
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -503,8 +535,8 @@ def run_ours(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     e0.record()
-    for _ in range(args.steps):
-        step()
+    for i in range(args.steps):
+        step(i)
     e1.record()
     torch.cuda.synchronize()
     ms_total = e0.elapsed_time(e1)
@@ -571,13 +603,7 @@ def run_ours(args):
         "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": round(ms_step, 5), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": "even-odd Wilson-clover Dslash (Mhat_ee apply = 2 fused hop launches), 32^3x64, fp32, "
-                               "12-real links, kappa 0.1355, csw 1.0, eps 0.5 (BASELINE.json configs[3] lattice, "
-                               "north_star 70% target workload)",
-                   "dims": list(dims), "reconstruct": 12, "kappa": KAPPA, "csw": CSW, "eps": EPS,
-                   "parallelism": "replicas only (x%d)" % world,
-                   "l2": "inputs larger than L2: gauge 403 MB + clover 604 MB + spinors 302 MB per step",
-                   "flop_per_step": step_flops(Vh), "gauge_recipe": "32^3x16 block of the configs[0] recipe tiled 4x in t"},
+        "config": workload_config(world),
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
     }
     if not args.no_cpu_baseline:
@@ -588,7 +614,7 @@ def run_ours(args):
             line["cg"] = solver_table(c, w)
             del w
             torch.cuda.empty_cache()
-            line["configs"] = config_table(c, peak, args.config4, cheb_degree=args.cheb_degree)
+            line["configs"] = config_table(c, peak, not args.no_config4, cheb_degree=args.cheb_degree)
     if args.config4_only and rank == 0:
         del w
         torch.cuda.empty_cache()
@@ -599,10 +625,32 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def spawn_replicas(args):
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves, the way the driver
+    does (one process per GPU, torch.distributed.run on 127.0.0.1), and pass rank 0's JSON line through."""
+    import socket
+    import subprocess
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        raise SystemExit("bench.py: --gpus %d asked for, %d CUDA device(s) visible" % (args.gpus, have))
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    raise SystemExit(subprocess.call(replica_command(args.gpus, port, sys.argv[1:])))
+
+
+def replica_command(ngpus, port, argv):
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(ngpus),
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+
+
 if __name__ == "__main__":
     a = parse_args()
     TABLE_SCALE = a.table_scale
     if a.impl == "reference":
         run_reference(a)
+    elif a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_replicas(a)
     else:
         run_ours(a)

@@ -290,6 +290,7 @@ __device__ __forceinline__ void clover_apply(T (&o)[24], const T* __restrict__ c
 template <typename T> struct Neighbours {
     int xp, xm, yp, ym, zp, zm, tp, tm;
     T sgn_tp, sgn_tm;
+    __device__ __forceinline__ Neighbours() {} /* filled in by the caller (hop_tile.cu: staged slots instead of cb) */
     __device__ __forceinline__ Neighbours(const DevGeom& g, int cb, int parity, T tb)
     {
         const Coord c = cb_to_coord(g, cb, parity);

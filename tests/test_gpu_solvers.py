@@ -374,3 +374,36 @@ def test_solver_entry_points_reject_wrong_precision_handles():
     with pytest.raises(qcd.QcdError) as e:
         c.set_operator(g64, g64, None, None, kappa, 0.0, 2)       # g_lo must be fp32 or 16-bit
     assert e.value.code == qcd.EINVAL
+
+
+@pytest.mark.parametrize("dims,variant", [((8, 8, 8, 16), "40"), ((16, 8, 4, 4), "40"), ((16, 8, 4, 4), "41"), ((16, 4, 2, 2), "32")])
+def test_chebyshev_multi_rhs_tiled_kernel_matches_oracle(dims, variant, monkeypatch):
+    """The opt-in shared-memory tile kernel (hop_tile.cu; north_star (2) "neighbour spinors staged
+    through shared memory"): rows of a 4-D tile staged with cp.async, faces read directly.  Both tile
+    shapes ((4,4,4,2) for X/2 = 4, (8,4,2,2) for X/2 = 8), tiles that span a whole extent (wrap onto
+    themselves), 5 vectors on 4 (3) groups, against the oracle and against the default kernel."""
+    c = ctx()
+    kappa, scale, nvec = 0.2, 2.6, 5
+    U, g, _, _, _ = setup_operator(c, dims, kappa, 0.0, 4, 12)
+    coeff = inputs.chebyshev_sign_coefficients(12)
+    vs = [inputs.round_to_f32(inputs.spinor_field(dims, 0, 40 + i)) for i in range(nvec)]
+    batch = torch.cat([pack(c, v, dims, 4) for v in vs])
+    y, y0 = torch.empty_like(batch), torch.empty_like(batch)
+    c.ensure_workspace(2 * batch.numel() * 4)
+    monkeypatch.setenv("QCD_MRHS_TILE", "0")
+    n0 = c.launch_count()
+    c.cheb_apply_multi(y0, batch, nvec, g, kappa, coeff, scale)
+    monkeypatch.setenv("QCD_MRHS_TILE", "1")
+    monkeypatch.setenv("QCD_MRHS_VARIANT", variant)
+    c.cheb_apply_multi(y, batch, nvec, g, kappa, coeff, scale)
+    n = batch.numel() // nvec
+    for i, v in enumerate(vs):
+        want = orc.cheb(v, U, dims, kappa, coeff, scale)
+        assert relerr(unpack(c, y[i * n:(i + 1) * n].contiguous(), dims), want) <= TOL[4]
+    assert relerr(y.cpu().numpy(), y0.cpu().numpy()) <= 1e-6
+    out = torch.empty_like(batch)
+    c.wilson_multi(out, batch, nvec, g, kappa, True)
+    monkeypatch.setenv("QCD_MRHS_TILE", "0")
+    out0 = torch.empty_like(batch)
+    c.wilson_multi(out0, batch, nvec, g, kappa, True)
+    assert relerr(out.cpu().numpy(), out0.cpu().numpy()) <= 1e-6

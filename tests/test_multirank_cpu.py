@@ -58,3 +58,20 @@ def test_reference_arm_prints_on_rank0_only():
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["metric"] == "wilson_clover_dslash_gflops"
+
+
+def test_gpus_flag_spawns_one_rank_per_gpu_on_localhost():
+    """`bench.py --gpus N` without a launcher starts its own N ranks (it used to run
+    one replica and print n_gpus: 1); without N devices it refuses instead of under-reporting."""
+    import argparse
+    import pytest
+    sys.path.insert(0, ROOT)
+    import bench
+    cmd = bench.replica_command(4, 29511, ["--gpus", "4", "--steps", "7"])
+    assert cmd[1:3] == ["-m", "torch.distributed.run"]
+    assert "--nproc-per-node" in cmd and cmd[cmd.index("--nproc-per-node") + 1] == "4"
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1"
+    assert cmd[-4:] == ["--gpus", "4", "--steps", "7"] and cmd[-5].endswith("bench.py")
+    with pytest.raises(SystemExit) as e:
+        bench.spawn_replicas(argparse.Namespace(gpus=1024))
+    assert "1024" in str(e.value)
