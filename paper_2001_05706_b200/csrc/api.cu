@@ -293,6 +293,12 @@ static int apply_full(qcd_ctx* ctx, void* out, const void* in, const qcd_gauge* 
                 L.norm_out = p == 0 ? ex->norm_tmp : ex->norm_out;
                 L.norm_add = p == 0 ? nullptr : ex->norm_tmp;
             }
+            if (ex->cg_r) { /* each launch updates its parity block of r; the second one decides */
+                L.cg_r = (char*)ex->cg_r + p * blk;
+                L.cg_num = ex->cg_num; L.cg_den = ex->cg_den;
+                L.cg_ctl = p == 1 ? ex->cg_ctl : nullptr;
+                L.cg_status = p == 1 ? ex->cg_status : nullptr;
+            }
         }
         L.out = (char*)out + p * blk;
         L.in = (const char*)in + (1 - p) * blk;
@@ -321,7 +327,10 @@ static int apply_eo(qcd_ctx* ctx, void* out, const void* in, void* tmp, const qc
     int rc = hop_launch(ctx, g, L);
     if (rc) return rc;
     memset(&L, 0, sizeof(L));
-    if (ex) { L.halt = ex->halt; L.norm_out = ex->norm_out; }
+    if (ex) {
+        L.halt = ex->halt; L.norm_out = ex->norm_out;
+        L.cg_r = ex->cg_r; L.cg_num = ex->cg_num; L.cg_den = ex->cg_den; L.cg_ctl = ex->cg_ctl; L.cg_status = ex->cg_status;
+    }
     L.out = out; L.in = tmp; L.z = in; L.a = 1.0; L.b = -kappa * kappa; L.out_parity = p; L.dagger = dagger;
     if (c) { L.mode = HOP_CLOVER_Z; L.clover = (const char*)c->data + p * c->block_bytes; }
     else L.mode = HOP_XPAY;

@@ -113,13 +113,7 @@ __global__ void __launch_bounds__(BLAS_THREADS) cg_update_kernel(DevScalar a, co
         if (halted(&ctl->halt)) return;
         /* breakdown (reading O6: <p,Np> <= 0 or NaN) is detected before anything is written */
         if (a.num && !(*a.den > 0.0)) {
-            if (blockIdx.x == 0 && threadIdx.x == 0) {
-                ctl->halt = CG_BREAKDOWN;
-                if (status) {
-                    reinterpret_cast<volatile int*>(status)[1] = CG_BREAKDOWN;
-                    __threadfence_system();
-                }
-            }
+            if (blockIdx.x == 0 && threadIdx.x == 0) cg_flag_breakdown(ctl, status);
             return;
         }
     }
@@ -148,27 +142,42 @@ __global__ void __launch_bounds__(BLAS_THREADS) cg_update_kernel(DevScalar a, co
     double tot;
     if (grid_sum(s, partial, ticket, &tot)) {
         *out = tot;
-        if (ctl) {
-            /* the stopping test of reading O6 / the update rule of reading O7, taken on the device */
-            const double rn = sqrt(tot);
-            const int it = ctl->iter + 1;
-            int h = CG_RUN;
-            ctl->rnorm = rn;
-            ctl->iter = it;
-            if (ctl->delta > 0.0) {
-                double rm = ctl->rmax;
-                if (rn > rm) { rm = rn; ctl->rmax = rm; }
-                if (rn < ctl->delta * rm || rn <= ctl->thresh) h = CG_UPDATE_DUE;
-            } else if (rn <= ctl->thresh) {
-                h = CG_CONVERGED;
-            }
-            if (h) ctl->halt = h;
-            if (status) {
-                volatile int* hs = reinterpret_cast<volatile int*>(status);
-                hs[1] = h;
-                __threadfence_system();
-                hs[0] = it;
-            }
+        if (ctl) cg_decide(ctl, status, tot); /* stopping test (O6) / update rule (O7), taken on the device */
+    }
+}
+
+/* The other half of a CG iteration whose residual update ran in the epilogue of the last hop launch
+ * (hop_kernel.cuh, HopArgs::cg_r):  x += alpha p ; p = r + beta p.  `iter` is the iteration the host
+ * enqueued this launch for.  While the solver runs (halt == 0) both updates are done.  In the iteration
+ * that halted it (converged, or reliable update due: ctl->iter == iter) only x += alpha p is (readings
+ * O6 / O7: the stop test and the update decision come after the x update and before the p update);
+ * launches enqueued for later iterations, and everything after a breakdown, do nothing. */
+template <typename T>
+__global__ void __launch_bounds__(BLAS_THREADS) cg_xp_kernel(DevScalar a, DevScalar b, const T* __restrict__ r, T* __restrict__ x, T* __restrict__ p, size_t nvec, const CgCtl* ctl,
+                             int iter)
+{
+    typedef typename Vec<T>::type V;
+    const int h = *reinterpret_cast<const volatile int*>(&ctl->halt);
+    if (h == CG_BREAKDOWN || (h != CG_RUN && ctl->iter != iter)) return;
+    const bool pupd = (h == CG_RUN);
+    const T aa = (T)eval(a), bb = pupd ? (T)eval(b) : (T)0;
+    const V* rv = reinterpret_cast<const V*>(r);
+    V* xv = reinterpret_cast<V*>(x);
+    V* pv = reinterpret_cast<V*>(p);
+#pragma unroll BLAS_UNROLL_N
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
+        T ps[Vec<T>::reals], xs[Vec<T>::reals];
+        vec_get(pv[i], ps);
+        vec_get(xv[i], xs);
+#pragma unroll
+        for (int k = 0; k < Vec<T>::reals; k++) xs[k] += aa * ps[k];
+        xv[i] = vec_make(xs);
+        if (pupd) {
+            T rs[Vec<T>::reals];
+            vec_get(rv[i], rs);
+#pragma unroll
+            for (int k = 0; k < Vec<T>::reals; k++) ps[k] = rs[k] + bb * ps[k];
+            pv[i] = vec_make(ps);
         }
     }
 }
@@ -373,6 +382,18 @@ int blas_cg_update(qcd_ctx* ctx, DevScalar a, const void* p, const void* q, void
                                                                                     ctx->d_partial, ctx->d_ticket, d_out, ctl, status);
     }
     return check_launch(ctx, "cg_update");
+}
+
+int blas_cg_xp(qcd_ctx* ctx, DevScalar a, DevScalar b, const void* r, void* x, void* p, size_t nreal, int prec, const CgCtl* ctl, int iter)
+{
+    if (prec == 4) {
+        const size_t nv = nreal / 4;
+        cg_xp_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, b, (const float*)r, (float*)x, (float*)p, nv, ctl, iter);
+    } else {
+        const size_t nv = nreal / 2;
+        cg_xp_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, b, (const double*)r, (double*)x, (double*)p, nv, ctl, iter);
+    }
+    return check_launch(ctx, "cg_xp");
 }
 
 int blas_accumulate_hi(qcd_ctx* ctx, void* y_hi, void* x_lo, size_t nreal, size_t Vh)

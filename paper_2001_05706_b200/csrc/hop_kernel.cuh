@@ -41,6 +41,12 @@ template <typename T> struct HopArgs {
     const double* norm_add;
     double* norm_partial;   /* one slot per block                                              */
     unsigned int* norm_ticket;
+    /* CG residual update fused into the epilogue (HopLaunch::cg_r) */
+    T* cg_r;
+    const double* cg_num;
+    const double* cg_den;
+    CgCtl* cg_ctl;
+    int* cg_status;
 };
 
 /* |v|^2 of the block's sites, accumulated in fp64, one partial per block; the last block to
@@ -85,7 +91,21 @@ __device__ __forceinline__ void hop_fused_norm(const HopArgs<T>& A, const T (&v)
 #pragma unroll
         for (int i = 0; i < THREADS / 32; i++) b += sm[i];
         *A.norm_out = b;
+        if (A.cg_ctl) cg_decide(A.cg_ctl, A.cg_status, b);
     }
+}
+
+/* epilogue of the launch that computes q = (M^dag M p)(x) for this site: r -= alpha q in place of
+ * storing q, alpha = cg_num / cg_den rounded to T (reading O6; O7: alpha = (float)(rho / <p,Np>)) */
+template <typename T>
+__device__ __forceinline__ void hop_cg_residual(const HopArgs<T>& A, T (&q)[24], size_t Vh, size_t cb, bool active)
+{
+    const T alpha = (T)(*A.cg_num / *A.cg_den);
+    T rr[24];
+    load_planes_rw<T, 24>(rr, A.cg_r, Vh, cb);
+#pragma unroll
+    for (int i = 0; i < 24; i++) q[i] = rr[i] - alpha * q[i];
+    if (active) store_planes<T, 24>(A.cg_r, Vh, cb, q);
 }
 
 /* ---- where a neighbour spinor comes from ---------------------------------------------- */
@@ -343,6 +363,11 @@ template <typename T, int RECON, int DAG, int MODE>
 __global__ void __launch_bounds__(HOP_THREADS, (sizeof(T) == 4 ? HOP_MINBLOCKS_F32 : HOP_MINBLOCKS_F64) * 128 / HOP_THREADS) hop_kernel(const HopArgs<T> A)
 {
     if (A.halt && *reinterpret_cast<const volatile int*>(A.halt) != 0) return;
+    const bool fuse_cg = (MODE == HOP_XPAY || MODE == HOP_CLOVER_Z) && A.cg_r != nullptr;
+    if (fuse_cg && !(*A.cg_den > 0.0)) { /* breakdown: nothing is written */
+        if (A.cg_ctl && blockIdx.x == 0 && threadIdx.x == 0) cg_flag_breakdown(A.cg_ctl, A.cg_status);
+        return;
+    }
     int cb = blockIdx.x * blockDim.x + threadIdx.x;
     const bool want_norm = (MODE == HOP_XPAY || MODE == HOP_CLOVER_Z) && A.norm_out != nullptr;
     const bool active = cb < A.geo.Vh;
@@ -364,7 +389,8 @@ __global__ void __launch_bounds__(HOP_THREADS, (sizeof(T) == 4 ? HOP_MINBLOCKS_F
         load_planes_rw<T, 24>(zz, A.z, Vh, (size_t)cb);
 #pragma unroll
         for (int i = 0; i < 24; i++) acc[i] = A.a * zz[i] + A.b * acc[i];
-        if (active) store_planes<T, 24>(A.out, Vh, (size_t)cb, acc);
+        if (fuse_cg) hop_cg_residual<T>(A, acc, Vh, (size_t)cb, active);
+        else if (active) store_planes<T, 24>(A.out, Vh, (size_t)cb, acc);
         if (want_norm) hop_fused_norm<T, HOP_THREADS>(A, acc, active);
     } else if (MODE == HOP_CLOVER_Z) {
         T zz[24], az[24];
@@ -372,7 +398,8 @@ __global__ void __launch_bounds__(HOP_THREADS, (sizeof(T) == 4 ? HOP_MINBLOCKS_F
         clover_apply<T>(az, A.clover, Vh, (size_t)cb, zz);
 #pragma unroll
         for (int i = 0; i < 24; i++) acc[i] = A.a * az[i] + A.b * acc[i];
-        if (active) store_planes<T, 24>(A.out, Vh, (size_t)cb, acc);
+        if (fuse_cg) hop_cg_residual<T>(A, acc, Vh, (size_t)cb, active);
+        else if (active) store_planes<T, 24>(A.out, Vh, (size_t)cb, acc);
         if (want_norm) hop_fused_norm<T, HOP_THREADS>(A, acc, active);
     } else if (MODE == HOP_CLOVER_OUT) {
         T o[24];
@@ -563,6 +590,11 @@ template <typename T> static HopArgs<T> make_hop_args(const qcd_gauge* g, const 
     A.norm_add = L.norm_add;
     A.norm_partial = g->ctx->d_hop_partial;
     A.norm_ticket = g->ctx->d_ticket + 1; /* slot 0 belongs to blas.cu, 8 to clover.cu */
+    A.cg_r = (T*)L.cg_r;
+    A.cg_num = L.cg_num;
+    A.cg_den = L.cg_den;
+    A.cg_ctl = L.cg_ctl;
+    A.cg_status = L.cg_status;
     return A;
 }
 

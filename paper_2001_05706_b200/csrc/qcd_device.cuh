@@ -169,6 +169,43 @@ __device__ __forceinline__ void store_link(T* block, size_t Vh, size_t cb, const
     }
 }
 
+/* ---- solver control on the device -------------------------------------
+ * Called by ONE thread once the new |r|^2 of an iteration is known (the last block of the CG
+ * update kernel, or of the hop launch with the residual update fused into its epilogue): counts
+ * the iteration, takes the stopping test of reading O6 or the reliable-update rule of reading O7,
+ * sets ctl->halt and mirrors (iterations done, halt) to the mapped host words the solver polls. */
+__device__ __forceinline__ void cg_decide(CgCtl* ctl, int* status, double rho_new)
+{
+    const double rn = sqrt(rho_new);
+    const int it = ctl->iter + 1;
+    int h = CG_RUN;
+    ctl->rnorm = rn;
+    ctl->iter = it;
+    if (ctl->delta > 0.0) {
+        double rm = ctl->rmax;
+        if (rn > rm) { rm = rn; ctl->rmax = rm; }
+        if (rn < ctl->delta * rm || rn <= ctl->thresh) h = CG_UPDATE_DUE;
+    } else if (rn <= ctl->thresh) {
+        h = CG_CONVERGED;
+    }
+    if (h) ctl->halt = h;
+    if (status) {
+        volatile int* hs = reinterpret_cast<volatile int*>(status);
+        hs[1] = h;
+        __threadfence_system();
+        hs[0] = it;
+    }
+}
+/* breakdown (reading O6: <p,Np> <= 0 or NaN): flagged by one thread before anything is written */
+__device__ __forceinline__ void cg_flag_breakdown(CgCtl* ctl, int* status)
+{
+    ctl->halt = CG_BREAKDOWN;
+    if (status) {
+        reinterpret_cast<volatile int*>(status)[1] = CG_BREAKDOWN;
+        __threadfence_system();
+    }
+}
+
 /* ---- checkerboard indexing (reading S3) -------------------------------------------
  * lexicographic s = x + X (y + Y (z + Z t)); parity = (x+y+z+t)&1; cb = s >> 1. */
 struct DevGeom {

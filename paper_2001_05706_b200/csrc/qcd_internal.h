@@ -124,6 +124,15 @@ struct HopLaunch {
     const int* halt;      /* device flag: the launch does nothing while *halt != 0 (NULL = always run) */
     double* norm_out;     /* device: receives |out|^2 (+ *norm_add), accumulated in fp64 in the epilogue (modes 1,2) */
     const double* norm_add;
+    /* CG residual update fused into the epilogue (modes 1,2): with q the value this launch computes for a site,
+     *   r -= (cg_num / cg_den) q ;  norm_out = |r|^2 (+ *norm_add) ;  q itself is not stored.
+     * A denominator that is not > 0 makes the launch flag a breakdown and write nothing.  With cg_ctl the
+     * last block counts the iteration and takes the stop / reliable-update decision (cg_decide). */
+    void* cg_r;           /* one-parity block of the residual, same precision as out */
+    const double* cg_num;
+    const double* cg_den;
+    CgCtl* cg_ctl;
+    int* cg_status;
     const void* in;       /* other-parity block                                   */
     const void* z;        /* own-parity block (modes 1,2,4)                       */
     const void* tm;       /* cheb: b_{k+2}, own parity (may alias out)            */
@@ -145,6 +154,13 @@ struct OpExtra {
     const int* halt;   /* gate (see HopLaunch)                                                  */
     double* norm_out;  /* device: |out|^2 of the whole result, fused into the launch(es) writing it */
     double* norm_tmp;  /* device scratch double (full-lattice form: partial result of the first launch) */
+    /* residual update fused into the launch(es) that would write `out` (see HopLaunch::cg_r): r is a field
+     * shaped like out; norm_out then receives |r|^2 and out is not written */
+    void* cg_r;
+    const double* cg_num;
+    const double* cg_den;
+    CgCtl* cg_ctl;
+    int* cg_status;
 };
 int op_apply_M(qcd_ctx* ctx, void* out, const void* in, void* tmp, const qcd_gauge* g, const qcd_clover* c,
                double kappa, int parity, int dagger, const OpExtra* ex = nullptr);
@@ -181,6 +197,8 @@ int blas_redot(qcd_ctx*, const void* x, const void* y, size_t nreal, int prec, d
  * (CgCtl) and mirrors (iter, halt) to the mapped host words `status`. */
 int blas_cg_update(qcd_ctx*, DevScalar a, const void* p, const void* q, void* x, void* r,
                    size_t nreal, int prec, double* d_out, CgCtl* ctl = nullptr, int* status = nullptr);
+/* x += a p; and, unless the solver halted in iteration `iter`, p = r + b p (see blas.cu) */
+int blas_cg_xp(qcd_ctx*, DevScalar a, DevScalar b, const void* r, void* x, void* p, size_t nreal, int prec, const CgCtl* ctl, int iter);
 /* y(hi) += x(lo); x = 0 */
 int blas_accumulate_hi(qcd_ctx*, void* y_hi, void* x_lo, size_t nreal, size_t Vh);
 /* r_hi = b - t (fp64); r_lo = (float) r_hi; *d_out = |r_hi|^2; with ctl: rmax = |r_hi|,

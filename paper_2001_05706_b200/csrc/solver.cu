@@ -14,6 +14,12 @@
 
 #include "qcd_internal.h"
 
+#define RC(expr)               \
+    do {                       \
+        int rc__ = (expr);     \
+        if (rc__) return rc__; \
+    } while (0)
+
 namespace {
 
 qcd_ctx* g_last_ctx = nullptr;
@@ -53,18 +59,32 @@ int apply_N(const Op& o, void* q, const void* p, void* t, void* tmp, const OpExt
     return op_apply_M(o.ctx, q, t, tmp, o.g, o.c, o.kappa, o.parity, 1, ex ? &gate : nullptr);
 }
 
+/* One CG iteration n on the device, the BLAS fused into the operator (SURVEY.md 8(a) a10 "fused CG BLAS"):
+ *   t = M p, <p,Np> = |t|^2 in the epilogue of the launch writing t;
+ *   q = M^dag t is never stored: the launch that computes it does r -= alpha q, rho' = |r|^2 and the stop /
+ *   reliable-update decision (cg_decide) in its epilogue;
+ *   x += alpha p ; p = r + beta p in one pass (blas_cg_xp), the p update only while the solver runs.
+ * Per iteration and site this moves 3 vectors less than separate  |t|^2, (x, r, rho') and p passes. */
+int cg_iteration(const Op& o, int n, void* x, void* r, void* p, void* q, void* t, void* tmp)
+{
+    qcd_ctx* ctx = o.ctx;
+    double* d = ctx->d_scalar;
+    double *rho = d + rho_slot(n - 1), *rho2 = d + rho_slot(n);
+    const int* halt = &ctx->d_ctl->halt;
+    const int P = o.g->precision;
+    const OpExtra ex1 = {halt, d + S_PQ, d + S_NTMP};
+    RC(op_apply_M(ctx, t, p, tmp, o.g, o.c, o.kappa, o.parity, 0, &ex1));
+    const OpExtra ex2 = {halt, rho2, d + S_NTMP, r, rho, d + S_PQ, ctx->d_ctl, ctx->d_status};
+    RC(op_apply_M(ctx, q, t, tmp, o.g, o.c, o.kappa, o.parity, 1, &ex2));
+    return blas_cg_xp(ctx, dev_ratio(rho, d + S_PQ), dev_ratio(rho2, rho), r, x, p, o.nreal, P, ctx->d_ctl, n);
+}
+
 int fetch(qcd_ctx* ctx, int slot, int n)
 {
     QCD_CHECK_CUDA(cudaMemcpyAsync(ctx->h_scalar + slot, ctx->d_scalar + slot, sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream));
     QCD_CHECK_CUDA(cudaStreamSynchronize(ctx->stream));
     return QCD_OK;
 }
-
-#define RC(expr)               \
-    do {                       \
-        int rc__ = (expr);     \
-        if (rc__) return rc__; \
-    } while (0)
 
 /* ---- device-side control (CgCtl) ----------------------------------------------------------
  * The host enqueues iterations ahead of the device; the CG update kernel decides on the device
@@ -112,7 +132,10 @@ int run_ahead()
     /* iterations the host may be ahead of the device; each one enqueued past a halt costs a few
      * skipped launches, each one less risks an idle device */
     const char* e = getenv("QCD_CG_RUNAHEAD"); /* read per solve: tests sweep it */
-    int d = e ? atoi(e) : 1; /* measured on B200, 32^3x64: 0, 1, 2 within noise; 4 and 8 slower (launches skipped after every reliable update) */
+    int d = e ? atoi(e) : 0; /* 0: enqueue iteration n + 1 as soon as iteration n's residual update has reported (the x / p pass of
+                               * iteration n is still running then, so the device never idles); measured on B200, 32^3x64: mixed CG 56.7 /
+                               * 57.7 / 58.2 ms for 0 / 1 / 2 (every launch enqueued past a reliable update is a skipped launch), pure
+                               * fp64 CG 92.4 - 93.0 ms for all three */
     if (d < 0) d = 0;
     if (d > 64) d = 64;
     return d;
@@ -152,17 +175,11 @@ int cg_pure(qcd_ctx* ctx, void* x, const void* b, double tol, int maxiter, qcd_s
     int k = 0, conv = (bnorm == 0.0), brk = 0;
     if (!conv && maxiter > 0) {
         RC(ctl_start(ctx, tol * bnorm, 0.0, bnorm));
-        const int* halt = &ctx->d_ctl->halt;
-        const OpExtra ex = {halt, d + S_PQ, d + S_NTMP};
         const int ahead = run_ahead();
         int n = 0;
         while (n < maxiter) {
             n++;
-            double *rho = d + rho_slot(n - 1), *rho2 = d + rho_slot(n);
-            /* <p, N p> = |M p|^2, accumulated while t = M p is written */
-            RC(apply_N(o, q, p, t, tmp, &ex));
-            RC(blas_cg_update(ctx, dev_ratio(rho, d + S_PQ), p, q, x, r, o.nreal, P, rho2, ctx->d_ctl, ctx->d_status));
-            RC(blas_axpby(ctx, host_scalar(1.0), r, dev_ratio(rho2, rho), p, o.nreal, P, halt)); /* p = r + beta p */
+            RC(cg_iteration(o, n, x, r, p, q, t, tmp));
             if (n > ahead) RC(ctl_wait(ctx, n - ahead));
             if (ctx->h_status[1]) break;
         }
@@ -222,25 +239,23 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
     if (!conv && maxiter > 0) {
         RC(ctl_start(ctx, tol * bnorm, ctx->delta, sqrt(h[rho_slot(0)])));
         const int* halt = &ctx->d_ctl->halt;
-        const OpExtra ex = {halt, d + S_PQ, d + S_NTMP};
         const int ahead = run_ahead();
         int nq = 0; /* iterations enqueued (== executed whenever the device is not halted) */
         for (;;) {
             while (nq < maxiter) {
                 nq++;
-                double *rho = d + rho_slot(nq - 1), *rho2 = d + rho_slot(nq);
                 if (half) {
+                    double *rho = d + rho_slot(nq - 1), *rho2 = d + rho_slot(nq);
                     /* q = M^dag store16(M store16(p)); <p, q> taken as written */
                     RC(op_apply_M_half(ctx, th16, 0, ph, tmp16, ol.g, ol.c, ol.kappa, ol.parity, 0, halt));
                     RC(op_apply_M_half(ctx, q, 1, th16, tmp16, ol.g, ol.c, ol.kappa, ol.parity, 1, halt));
                     RC(blas_redot(ctx, p, q, n, 4, d + S_PQ, halt));
+                    RC(blas_cg_update(ctx, dev_ratio(rho, d + S_PQ), p, q, x, r, n, 4, rho2, ctx->d_ctl, ctx->d_status));
+                    /* p = r + beta p, beta = (float)(rho'/rho); skipped when the update halted the iteration */
+                    RC(half_xpay_store(ctx, host_scalar(1.0), r, dev_ratio(rho2, rho), 0, p, ph, Vh, nblocks, halt));
                 } else {
-                    RC(apply_N(ol, q, p, tl, l2, &ex)); /* <p, N p> = |M p|^2 fused into the launch writing tl = M p */
+                    RC(cg_iteration(ol, nq, x, r, p, q, tl, l2));
                 }
-                RC(blas_cg_update(ctx, dev_ratio(rho, d + S_PQ), p, q, x, r, n, 4, rho2, ctx->d_ctl, ctx->d_status));
-                /* p = r + beta p, beta = (float)(rho'/rho); skipped when the update halted the iteration */
-                if (half) RC(half_xpay_store(ctx, host_scalar(1.0), r, dev_ratio(rho2, rho), 0, p, ph, Vh, nblocks, halt));
-                else RC(blas_axpby(ctx, host_scalar(1.0), r, dev_ratio(rho2, rho), p, n, 4, halt));
                 if (nq > ahead) RC(ctl_wait(ctx, nq - ahead));
                 if (ctx->h_status[1]) break;
             }
