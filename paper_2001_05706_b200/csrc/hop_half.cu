@@ -42,6 +42,10 @@ __device__ __forceinline__ void half_clover_apply(float (&o)[24], const unsigned
 #ifndef HOP_HALF_DEPTH
 #define HOP_HALF_DEPTH 1 /* directions whose loads are in flight ahead of the arithmetic */
 #endif
+/* Round 2, tried and dropped (profiles/hop_half_r2.md): a loop over mu with a 4-way switch around the projection and
+ * the spin reconstruction, two raw buffers in ping-pong (to bring the 50 KB body under the 32 KB instruction-cache
+ * level: ncu shows 0.66 - 0.9 warps per issue waiting for instructions).  ptxas then keeps part of the accumulator in
+ * local memory (600 - 830 B of spills, 164 LDL + 109 STL in the body) and the Wilson Mhat takes 359 us against 199 us. */
 
 /* The undecoded words of one direction: neighbour spinor (3 x int4 + norm) and link (int4 + int2),
  * 19 registers.  The 16-bit kernel moves half the bytes of the fp32 one per load instruction, so
@@ -88,25 +92,62 @@ __device__ __forceinline__ void half_int8x2(const int4& a, const int4& b, f2* o)
     half_int2x2(a.w, b.w, o[6], o[7]);
 }
 
+/* The 24 codes of the two sites' neighbour spinors as undecoded floats (packed_math.cuh,
+ * project2_codes): real index i = code i of the site = half (i & 1) of word i / 2.  The words are
+ * turned to offset binary (x = w ^ 0x80008000) and, for the lower spin components, also negated per
+ * 16-bit half in the integer domain (0x10000 - x: no half is 0, codes are clamped to +-32767, so no
+ * borrow crosses the halves); one PRMT drops a half into the mantissa of 2^23. */
+struct HalfCodes2 {
+    unsigned xa[12], xb[12], na[6], nb[6];
+    __device__ __forceinline__ HalfCodes2(const HalfRaw& ra, const HalfRaw& rb)
+    {
+        const int wa[12] = {ra.q0.x, ra.q0.y, ra.q0.z, ra.q0.w, ra.q1.x, ra.q1.y, ra.q1.z, ra.q1.w, ra.q2.x, ra.q2.y, ra.q2.z, ra.q2.w};
+        const int wb[12] = {rb.q0.x, rb.q0.y, rb.q0.z, rb.q0.w, rb.q1.x, rb.q1.y, rb.q1.z, rb.q1.w, rb.q2.x, rb.q2.y, rb.q2.z, rb.q2.w};
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            xa[k] = (unsigned)wa[k] ^ 0x80008000u;
+            xb[k] = (unsigned)wb[k] ^ 0x80008000u;
+        }
+#pragma unroll
+        for (int k = 0; k < 6; k++) {
+            na[k] = 0x10000u - xa[6 + k];
+            nb[k] = 0x10000u - xb[6 + k];
+        }
+    }
+    static __device__ __forceinline__ unsigned half_of(unsigned w, int hi) { return __byte_perm(w, 0x4B00u, hi ? 0x5432 : 0x5410); }
+    /* M + code i */
+    __device__ __forceinline__ f2 pos(int i) const { return f2_bits(half_of(xa[i >> 1], i & 1), half_of(xb[i >> 1], i & 1)); }
+    /* M - code i (i >= 12: only the lower spin components are ever wanted negated) */
+    __device__ __forceinline__ f2 neg(int i) const { return f2_bits(half_of(na[(i >> 1) - 6], i & 1), half_of(nb[(i >> 1) - 6], i & 1)); }
+};
+
 template <int MU, int DIR, int SG>
 __device__ __forceinline__ void half_compute_raw2(f2 (&acc)[24], const HalfRaw& ra, const HalfRaw& rb, f2 sign)
 {
-    f2 s[24], u[18], h[12], w[12];
-    half_int8x2(ra.q0, rb.q0, &s[0]);
-    half_int8x2(ra.q1, rb.q1, &s[8]);
-    half_int8x2(ra.q2, rb.q2, &s[16]);
+    f2 u[18], h[12], w[12];
     half_int8x2(ra.la, rb.la, &u[0]);
     half_int2x2(ra.lb.x, rb.lb.x, u[8], u[9]);
     half_int2x2(ra.lb.y, rb.lb.y, u[10], u[11]);
+    /* rows 0,1 stay codes (value x 32767), row 2 = conj(row0 x row1) of the codes (value x 32767^2) */
+    reconstruct_row2_2<false>(u, f2_set1(1.f));
+    const HalfCodes2 codes(ra, rb);
+    project2_codes<MU, SG>(h, codes);
     const f2 d = f2_set1(1.0f / 32767.0f);
-    reconstruct_row2_2(u, d);
-    project2<MU, SG>(h, s);
-    /* codes -> values once, on the colour-multiplied half spinor: norm / 32767 / 32767.  Here the
-     * division is a multiplication by the rounded reciprocal (one ulp, inside the arithmetic's own
-     * rounding); the format's exact n / 32767 is kept where stored values are read back as such. */
-    const f2 scale = sign * f2_make(ra.n, rb.n) * f2_set1((1.0f / 32767.0f) * (1.0f / 32767.0f));
-    colour_mul2<(DIR < 0)>(w, u, h, scale);
-    reconstruct_add2<MU, SG>(acc, w);
+    if (DIR < 0) {
+        /* U^dag mixes row 2 into every output: bring the colour-2 inputs to the scale of the others instead */
+        h[4] = h[4] * d; h[5] = h[5] * d; h[10] = h[10] * d; h[11] = h[11] * d;
+    }
+    colour_mul2<(DIR < 0), false>(w, u, h, d);
+    /* codes -> values once, folded into the accumulation: norm / 32767 / 32767 (the division is a
+     * multiplication by the rounded reciprocal: one ulp, inside the arithmetic's own rounding; the format's
+     * exact n / 32767 is kept where stored values are read back as such).  U h: colour 2 of the result
+     * comes from row 2 and carries one more factor 32767. */
+    const f2 s01 = sign * f2_make(ra.n, rb.n) * f2_set1((1.0f / 32767.0f) * (1.0f / 32767.0f));
+    const f2 s2 = DIR < 0 ? s01 : s01 * d;
+    const f2 sc[3] = {s01, s01, s2};
+    const f2 n01 = f2_neg(s01), n2 = DIR < 0 ? n01 : f2_neg(s2);
+    const f2 nsc[3] = {n01, n01, n2};
+    reconstruct_add2_scaled<MU, SG>(acc, w, sc, nsc);
 }
 
 /* the stored values code * (norm / 32767) of the two sites' spinors */

@@ -96,6 +96,45 @@ template <int MU, int S> __device__ __forceinline__ void project2(f2 (&h)[12], c
     }
 }
 
+/* The same projection taken straight from the UNDECODED 16-bit codes (hop_half.cu).  A code c sits in
+ * the low mantissa bits of a float as pos = M + c (M = 2^23 + 2^15) or, from the word negated in the
+ * integer domain, as neg = M - c.  Every h component is (upper code) +- (lower code), and both
+ *     pos(a) - pos(b) = c_a - c_b      and      pos(a) - neg(b) = c_a + c_b
+ * are exact in fp32: one packed subtraction per component replaces two decoding subtractions and the
+ * projection's own add (12 instead of 36 FMA-pipe instructions per direction). */
+template <int SG, typename Src> __device__ __forceinline__ f2 f2_pm_codes(const Src& src, int ia, int ib)
+{
+    return SG > 0 ? src.pos(ia) - src.neg(ib) : src.pos(ia) - src.pos(ib);
+}
+template <int MU, int S, typename Src> __device__ __forceinline__ void project2_codes(f2 (&h)[12], const Src& src)
+{
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int r0 = 2 * c, r1 = 2 * (3 + c), r2 = 2 * (6 + c), r3 = 2 * (9 + c);
+        if (MU == 0) {
+            h[r0] = f2_pm_codes<-S>(src, r0, r3 + 1);
+            h[r0 + 1] = f2_pm_codes<S>(src, r0 + 1, r3);
+            h[r1] = f2_pm_codes<-S>(src, r1, r2 + 1);
+            h[r1 + 1] = f2_pm_codes<S>(src, r1 + 1, r2);
+        } else if (MU == 1) {
+            h[r0] = f2_pm_codes<-S>(src, r0, r3);
+            h[r0 + 1] = f2_pm_codes<-S>(src, r0 + 1, r3 + 1);
+            h[r1] = f2_pm_codes<S>(src, r1, r2);
+            h[r1 + 1] = f2_pm_codes<S>(src, r1 + 1, r2 + 1);
+        } else if (MU == 2) {
+            h[r0] = f2_pm_codes<-S>(src, r0, r2 + 1);
+            h[r0 + 1] = f2_pm_codes<S>(src, r0 + 1, r2);
+            h[r1] = f2_pm_codes<S>(src, r1, r3 + 1);
+            h[r1 + 1] = f2_pm_codes<-S>(src, r1 + 1, r3);
+        } else {
+            h[r0] = f2_pm_codes<S>(src, r0, r2);
+            h[r0 + 1] = f2_pm_codes<S>(src, r0 + 1, r2 + 1);
+            h[r1] = f2_pm_codes<S>(src, r1, r3);
+            h[r1 + 1] = f2_pm_codes<S>(src, r1 + 1, r3 + 1);
+        }
+    }
+}
+
 /* ---- acc += rows 0..3 of (1 + S g_mu) chi from its upper half w (reconstruct_add) ----------- */
 template <int MU, int S> __device__ __forceinline__ void reconstruct_add2(f2 (&acc)[24], const f2 (&w)[12])
 {
@@ -131,10 +170,48 @@ template <int MU, int S> __device__ __forceinline__ void reconstruct_add2(f2 (&a
     }
 }
 
+/* acc += sc * (rows 0..3 of (1 + S g_mu) chi) with the scale folded into the accumulation: one fused
+ * multiply-add per term instead of a multiplication of w and an addition.  sc[c] / nsc[c] = the factor
+ * of colour component c and its negation (fma.f32x2 has no operand negation). */
+template <int MU, int S> __device__ __forceinline__ void reconstruct_add2_scaled(f2 (&acc)[24], const f2 (&w)[12], const f2 (&sc)[3], const f2 (&nsc)[3])
+{
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int j0 = 2 * c, j1 = 2 * (3 + c);
+        const int r2 = 2 * (6 + c), r3 = 2 * (9 + c);
+        const f2 p = S > 0 ? sc[c] : nsc[c], m = S > 0 ? nsc[c] : sc[c]; /* +S and -S times the scale */
+        acc[j0] = f2_fma(sc[c], w[j0], acc[j0]);
+        acc[j0 + 1] = f2_fma(sc[c], w[j0 + 1], acc[j0 + 1]);
+        acc[j1] = f2_fma(sc[c], w[j1], acc[j1]);
+        acc[j1 + 1] = f2_fma(sc[c], w[j1 + 1], acc[j1 + 1]);
+        if (MU == 0) {
+            acc[r2] = f2_fma(p, w[j1 + 1], acc[r2]);
+            acc[r2 + 1] = f2_fma(m, w[j1], acc[r2 + 1]);
+            acc[r3] = f2_fma(p, w[j0 + 1], acc[r3]);
+            acc[r3 + 1] = f2_fma(m, w[j0], acc[r3 + 1]);
+        } else if (MU == 1) {
+            acc[r2] = f2_fma(p, w[j1], acc[r2]);
+            acc[r2 + 1] = f2_fma(p, w[j1 + 1], acc[r2 + 1]);
+            acc[r3] = f2_fma(m, w[j0], acc[r3]);
+            acc[r3 + 1] = f2_fma(m, w[j0 + 1], acc[r3 + 1]);
+        } else if (MU == 2) {
+            acc[r2] = f2_fma(p, w[j0 + 1], acc[r2]);
+            acc[r2 + 1] = f2_fma(m, w[j0], acc[r2 + 1]);
+            acc[r3] = f2_fma(m, w[j1 + 1], acc[r3]);
+            acc[r3 + 1] = f2_fma(p, w[j1], acc[r3 + 1]);
+        } else {
+            acc[r2] = f2_fma(p, w[j0], acc[r2]);
+            acc[r2 + 1] = f2_fma(p, w[j0 + 1], acc[r2 + 1]);
+            acc[r3] = f2_fma(p, w[j1], acc[r3]);
+            acc[r3 + 1] = f2_fma(p, w[j1 + 1], acc[r3 + 1]);
+        }
+    }
+}
+
 /* ---- w_j = scale * U h_j (ADJ = 0) or scale * U^dag h_j (ADJ = 1), j = 0,1 (colour_mul) -----
  * re += ur hr - ui hi, im += ur hi + ui hr; U^dag takes conj(U_ba).  The subtraction runs on a
  * negated copy of the half spinor's imaginary (ADJ: real) parts: 6 negations per direction. */
-template <int ADJ> __device__ __forceinline__ void colour_mul2(f2 (&w)[12], const f2 (&u)[18], const f2 (&h)[12], f2 scale)
+template <int ADJ, bool SCALE = true> __device__ __forceinline__ void colour_mul2(f2 (&w)[12], const f2 (&u)[18], const f2 (&h)[12], f2 scale)
 {
     f2 n[6]; /* ADJ = 0: -Im h_{j,b} ; ADJ = 1: -Re h_{j,b} */
 #pragma unroll
@@ -161,13 +238,13 @@ template <int ADJ> __device__ __forceinline__ void colour_mul2(f2 (&w)[12], cons
                     im = f2_fma(ui, nn, im);
                 }
             }
-            w[2 * (3 * j + a)] = scale * re;
-            w[2 * (3 * j + a) + 1] = scale * im;
+            w[2 * (3 * j + a)] = SCALE ? scale * re : re;
+            w[2 * (3 * j + a) + 1] = SCALE ? scale * im : im;
         }
 }
 
 /* ---- row2 = d * conj(row0 x row1) (reconstruct_row2; reading S7), d a common factor --------- */
-__device__ __forceinline__ void reconstruct_row2_2(f2 (&u)[18], f2 d)
+template <bool SCALE = true> __device__ __forceinline__ void reconstruct_row2_2(f2 (&u)[18], f2 d)
 {
 #pragma unroll
     for (int c = 0; c < 3; c++) {
@@ -177,8 +254,8 @@ __device__ __forceinline__ void reconstruct_row2_2(f2 (&u)[18], f2 d)
         /* re = ar br - ai bi - cr dr + ci di ; im = ar bi + ai br - cr di - ci dr ; row2 = (re, -im) */
         const f2 p = f2_fma(ci, di, ar * br), q = f2_fma(cr, dr, ai * bi);
         const f2 r = f2_fma(ai, br, ar * bi), t = f2_fma(ci, dr, cr * di);
-        u[12 + 2 * c] = d * (p - q);
-        u[12 + 2 * c + 1] = d * (t - r);
+        u[12 + 2 * c] = SCALE ? d * (p - q) : p - q;
+        u[12 + 2 * c + 1] = SCALE ? d * (t - r) : t - r;
     }
 }
 
