@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--quick", action="store_true", help="skip the per-kernel / solver sections")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-solvers", action="store_true", help="kernel table only (for ncu passes)")
+    ap.add_argument("--solvers-only", action="store_true", help="headline step + solver table only (for ncu passes)")
     ap.add_argument("--config4", action="store_true", help="(default now) run the 48^3x96 Chebyshev workload (configs[4])")
     ap.add_argument("--no-config4", action="store_true", help="skip the 48^3x96 Chebyshev workload (configs[4])")
     ap.add_argument("--config4-only", action="store_true", help="only the configs[4] section (for ncu passes)")
@@ -333,7 +334,7 @@ def solver_table(c, w):
     x = torch.empty_like(b)
     out = {}
     c.ensure_workspace(c.workspace_bytes(dims, 8))
-    for name, lo in (("mixed_cg_q16_12/fp64_18", 2), ("mixed_cg_fp32_12/fp64_18", 1), ("cg_fp64_18", 0)):
+    for name, lo in (("cg_fp64_18", 0), ("mixed_cg_fp32_12/fp64_18", 1), ("mixed_cg_q16_12/fp64_18", 2)):
         if lo == 2:
             c.set_operator(w["g64"], w["g16"], w["c64"], w["c16"], KAPPA, CSW, 0, 0.1)
         elif lo:
@@ -608,7 +609,9 @@ def run_ours(args):
     }
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline()
-    if full:
+    if full and args.solvers_only:
+        line["cg"] = solver_table(c, w)
+    elif full:
         line["kernels"] = kernel_table(c, w, peak)
         if not args.no_solvers:
             line["cg"] = solver_table(c, w)

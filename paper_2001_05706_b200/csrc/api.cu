@@ -92,6 +92,7 @@ int qcd_finalize(qcd_ctx* c)
     if (c->d_ctl) cudaFree(c->d_ctl);
     if (c->h_status) cudaFreeHost((void*)c->h_status);
     if (c->d_hop_partial) cudaFree(c->d_hop_partial);
+    if (c->d_hop_ticket) cudaFree(c->d_hop_ticket);
     if (c->d_partial) cudaFree(c->d_partial);
     if (c->d_ticket) cudaFree(c->d_ticket);
     if (c->d_scalar) cudaFree(c->d_scalar);

@@ -49,49 +49,71 @@ template <typename T> struct HopArgs {
     int* cg_status;
 };
 
-/* |v|^2 of the block's sites, accumulated in fp64, one partial per block; the last block to
- * take a ticket sums the partials in block order (deterministic for a fixed grid) and writes
- * the result.  Called by every thread of the block (inactive threads pass active = false). */
+/* |v|^2 of the block's sites, accumulated in fp64.  Deterministic two-level reduction over the grid:
+ * every block writes its partial; the last block of each group of HOP_NORM_GROUP consecutive blocks to
+ * take the group's ticket sums that group's partials in index order into a group partial, then takes
+ * the top ticket, and the last group to do so sums the group partials in index order.  Which block does
+ * a sum varies from run to run, what it sums and in which order does not.  (A single last block summing
+ * all 16384 partials of a 32^3 x 64 launch with its 64 threads cost 21 us of tail per launch.)
+ * Called by every thread of the block (inactive threads pass active = false). */
+template <int THREADS> __device__ __forceinline__ double hop_block_sum(double s, double* sm)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads(); /* sm may still be read from the previous use */
+    if (l == 0) sm[w] = s;
+    __syncthreads();
+    double b = 0.0;
+#pragma unroll
+    for (int i = 0; i < THREADS / 32; i++) b += sm[i];
+    return b; /* the same value in every thread */
+}
+
 template <typename T, int THREADS>
 __device__ __forceinline__ void hop_fused_norm(const HopArgs<T>& A, const T (&v)[24], bool active)
 {
     __shared__ double sm[THREADS / 32];
-    __shared__ bool last;
+    __shared__ int role; /* 0: done, 1: last block of its group, 2: also last group */
     double s = 0.0;
     if (active) {
 #pragma unroll
         for (int i = 0; i < 24; i++) s += (double)v[i] * (double)v[i];
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-    if (l == 0) sm[w] = s;
-    __syncthreads();
+    const double b = hop_block_sum<THREADS>(s, sm);
+    const unsigned int nblocks = gridDim.x, ngroups = (nblocks + HOP_NORM_GROUP - 1) / HOP_NORM_GROUP;
+    const unsigned int grp = blockIdx.x / HOP_NORM_GROUP;
+    const unsigned int first = grp * HOP_NORM_GROUP;
+    const unsigned int members = min((unsigned int)HOP_NORM_GROUP, nblocks - first);
+    double* group_partial = A.norm_partial + nblocks;
     if (threadIdx.x == 0) {
-        double b = 0.0;
-#pragma unroll
-        for (int i = 0; i < THREADS / 32; i++) b += sm[i];
         A.norm_partial[blockIdx.x] = b;
         __threadfence();
-        const unsigned int t = atomicInc(A.norm_ticket, gridDim.x - 1); /* wraps back to 0 */
-        last = (t == gridDim.x - 1);
+        const unsigned int t = atomicInc(A.norm_ticket + 1 + grp, members - 1); /* wraps back to 0 */
+        role = (t == members - 1) ? 1 : 0;
     }
     __syncthreads();
-    if (!last) return;
+    if (role == 0) return;
+    __threadfence();
+    double g = 0.0;
+    for (unsigned int i = threadIdx.x; i < members; i += THREADS) g += __ldcg(A.norm_partial + first + i);
+    g = hop_block_sum<THREADS>(g, sm);
+    if (threadIdx.x == 0) {
+        group_partial[grp] = g;
+        __threadfence();
+        const unsigned int t = atomicInc(A.norm_ticket, ngroups - 1);
+        role = (t == ngroups - 1) ? 2 : 0;
+    }
+    __syncthreads();
+    if (role != 2) return;
     __threadfence();
     double t = 0.0;
-    for (unsigned int i = threadIdx.x; i < gridDim.x; i += THREADS) t += ((volatile double*)A.norm_partial)[i];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-    __syncthreads();
-    if (l == 0) sm[w] = t;
-    __syncthreads();
+    for (unsigned int i = threadIdx.x; i < ngroups; i += THREADS) t += __ldcg(group_partial + i);
+    t = hop_block_sum<THREADS>(t, sm);
     if (threadIdx.x == 0) {
-        double b = A.norm_add ? *A.norm_add : 0.0;
-#pragma unroll
-        for (int i = 0; i < THREADS / 32; i++) b += sm[i];
-        *A.norm_out = b;
-        if (A.cg_ctl) cg_decide(A.cg_ctl, A.cg_status, b);
+        const double tot = t + (A.norm_add ? *A.norm_add : 0.0);
+        *A.norm_out = tot;
+        if (A.cg_ctl) cg_decide(A.cg_ctl, A.cg_status, tot);
     }
 }
 
@@ -589,7 +611,7 @@ template <typename T> static HopArgs<T> make_hop_args(const qcd_gauge* g, const 
     A.norm_out = L.norm_out;
     A.norm_add = L.norm_add;
     A.norm_partial = g->ctx->d_hop_partial;
-    A.norm_ticket = g->ctx->d_ticket + 1; /* slot 0 belongs to blas.cu, 8 to clover.cu */
+    A.norm_ticket = g->ctx->d_hop_ticket; /* [0] the groups' ticket, [1 + g] group g's */
     A.cg_r = (T*)L.cg_r;
     A.cg_num = L.cg_num;
     A.cg_den = L.cg_den;

@@ -56,8 +56,10 @@ struct qcd_ctx {
     volatile int* h_status; /* mapped pinned host words written by the CG update kernel: [0] = iterations
                                executed, [1] = halt code; the host polls them instead of synchronising */
     int* d_status;          /* device address of h_status                  */
-    double* d_hop_partial;  /* per-block partials of the norm fused into the hop epilogue (grown on demand) */
-    size_t hop_partial_cap;
+    double* d_hop_partial;  /* norm fused into the hop epilogue: per-block partials, then one per group of
+                               HOP_NORM_GROUP blocks (grown on demand, hop_norm_scratch)               */
+    unsigned int* d_hop_ticket; /* one ticket per group + one for the groups, zero between launches   */
+    size_t hop_partial_cap;     /* blocks the scratch is sized for                                    */
     int max_blocks;
     int num_sms;
     long long launches;
@@ -146,6 +148,8 @@ struct HopLaunch {
 };
 
 int hop_launch(qcd_ctx* ctx, const qcd_gauge* g, const HopLaunch& L);
+enum { HOP_NORM_GROUP = 64 }; /* blocks per first-level group of the fused norm's reduction */
+int hop_norm_scratch(qcd_ctx* ctx, size_t nblocks); /* hop.cu: make the scratch of the fused norm hold nblocks blocks */
 void solver_forget_ctx(const qcd_ctx* ctx); /* solver.cu: qcd_finalize clears the "last ctx" of qcd_cg_solve */
 
 /* out = M in (or M^dag in): parity 2 = (A - kappa H) on the full lattice (two launches);

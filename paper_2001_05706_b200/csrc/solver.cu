@@ -343,17 +343,11 @@ int qcd_set_operator(qcd_ctx* ctx, const qcd_gauge* g_hi, const qcd_gauge* g_lo,
     ctx->kappa = kappa; ctx->csw = csw; ctx->op_parity = parity; ctx->delta = delta;
     ctx->op_set = 1;
     g_last_ctx = ctx;
+    /* size the scratch of the norm fused into the hop epilogue now, not inside a solve */
+    QCD_CHECK_CUDA(cudaSetDevice(ctx->device));
     {
-        /* size the per-block partials of the norm fused into the hop epilogue now, not inside a solve */
-        const size_t need = ((size_t)g_hi->geo.Vh + 63) / 64;
-        if (ctx->hop_partial_cap < need) {
-            QCD_CHECK_CUDA(cudaSetDevice(ctx->device));
-            if (ctx->d_hop_partial) cudaFree(ctx->d_hop_partial);
-            ctx->d_hop_partial = nullptr;
-            ctx->hop_partial_cap = 0;
-            QCD_CHECK_CUDA(cudaMalloc(&ctx->d_hop_partial, need * sizeof(double)));
-            ctx->hop_partial_cap = need;
-        }
+        const int rc = hop_norm_scratch(ctx, ((size_t)g_hi->geo.Vh + 63) / 64);
+        if (rc) return rc;
     }
     return QCD_OK;
 }
