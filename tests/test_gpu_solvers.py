@@ -58,12 +58,13 @@ def setup_operator(c, dims, kappa, csw, precision, recon, eps=0.5):
 
 
 @pytest.mark.parametrize("mode", [2, 0])
-@pytest.mark.parametrize("csw", [0.0, 1.0])
-def test_cg_fp64_matches_oracle(mode, csw):
-    """configs[2] at a size the oracle finishes in seconds (8^3 x 16; same eps, kappa, csw, tol)."""
+@pytest.mark.parametrize("csw,recon", [(0.0, 18), (1.0, 18), (1.0, 12)])
+def test_cg_fp64_matches_oracle(mode, csw, recon):
+    """configs[2] at a size the oracle finishes in seconds (8^3 x 16; same eps, kappa, csw, tol),
+    with 18-real fp64 links and with 12-real ones (row 2 rebuilt in fp64)."""
     c = ctx()
     dims, kappa, tol = (8, 8, 8, 16), 0.135, 1e-10
-    U, g, cl, A, Ainv = setup_operator(c, dims, kappa, csw, 8, 18)
+    U, g, cl, A, Ainv = setup_operator(c, dims, kappa, csw, 8, recon)
     b = inputs.spinor_field(dims, 0, 1)
     if mode != 2:
         b = b * (parity_mask(dims) == mode)
