@@ -314,7 +314,7 @@ cudaError_t hop_tile_launch_f32(const qcd_gauge* g, const HopLaunch& L, cudaStre
     *handled = false;
     if (L.mode != HOP_CHEB || L.nvec < 2 || g->reconstruct != 12) return cudaSuccess;
     const char* env = getenv("QCD_MRHS_TILE");
-    if (!env || atoi(env) == 0) return cudaSuccess;
+    if (!env || atoi(env) != 1) return cudaSuccess;
     const HopArgs<float> A = make_hop_args<float>(g, L);
     typedef Tile<8, 4, 2, 2> T8;
     typedef Tile<4, 4, 4, 2> T4;
