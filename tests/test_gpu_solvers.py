@@ -408,3 +408,23 @@ def test_chebyshev_multi_rhs_tiled_kernel_matches_oracle(dims, variant, monkeypa
     out0 = torch.empty_like(batch)
     c.wilson_multi(out0, batch, nvec, g, kappa, True)
     assert relerr(out.cpu().numpy(), out0.cpu().numpy()) <= 1e-6
+
+
+def test_cg_solve_after_finalize_of_its_ctx_is_an_error_not_a_crash():
+    """qcd_cg_solve uses the ctx that last called qcd_set_operator; once that ctx is finalised the call
+    must return QCD_EINVAL instead of touching freed memory."""
+    import ctypes as C
+    from paper_2001_05706_b200 import qcd
+    c2 = qcd.Context(0)
+    dims, kappa = (4, 4, 4, 4), 0.125
+    U = inputs.gauge_field(dims, 0.5, 0)
+    g = c2.gauge_load(to_dev(U, 8), dims, 8, 18, -1)
+    c2.ensure_workspace(c2.workspace_bytes(dims, 8))
+    c2.set_operator(g, None, None, None, kappa, 0.0, 2)
+    b = torch.randn(4 ** 4 * 24, device="cuda", dtype=torch.float64)
+    x = torch.empty_like(b)
+    assert qcd.lib().qcd_cg_solve(C.c_void_p(x.data_ptr()), C.c_void_p(b.data_ptr()), 1e-8, 500) == 0
+    torch.cuda.synchronize()
+    c2.close()
+    rc = qcd.lib().qcd_cg_solve(C.c_void_p(x.data_ptr()), C.c_void_p(b.data_ptr()), 1e-8, 500)
+    assert rc == qcd.EINVAL
