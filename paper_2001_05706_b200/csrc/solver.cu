@@ -55,7 +55,7 @@ int apply_N(const Op& o, void* q, const void* p, void* t, void* tmp, const OpExt
 {
     int rc = op_apply_M(o.ctx, t, p, tmp, o.g, o.c, o.kappa, o.parity, 0, ex);
     if (rc) return rc;
-    OpExtra gate = {ex ? ex->halt : nullptr, nullptr, nullptr};
+    OpExtra gate = {ex ? ex->halt : nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     return op_apply_M(o.ctx, q, t, tmp, o.g, o.c, o.kappa, o.parity, 1, ex ? &gate : nullptr);
 }
 
@@ -72,7 +72,7 @@ int cg_iteration(const Op& o, int n, void* x, void* r, void* p, void* q, void* t
     double *rho = d + rho_slot(n - 1), *rho2 = d + rho_slot(n);
     const int* halt = &ctx->d_ctl->halt;
     const int P = o.g->precision;
-    const OpExtra ex1 = {halt, d + S_PQ, d + S_NTMP};
+    const OpExtra ex1 = {halt, d + S_PQ, d + S_NTMP, nullptr, nullptr, nullptr, nullptr, nullptr};
     RC(op_apply_M(ctx, t, p, tmp, o.g, o.c, o.kappa, o.parity, 0, &ex1));
     const OpExtra ex2 = {halt, rho2, d + S_NTMP, r, rho, d + S_PQ, ctx->d_ctl, ctx->d_status};
     RC(op_apply_M(ctx, q, t, tmp, o.g, o.c, o.kappa, o.parity, 1, &ex2));
