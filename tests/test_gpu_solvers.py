@@ -428,3 +428,40 @@ def test_cg_solve_after_finalize_of_its_ctx_is_an_error_not_a_crash():
     c2.close()
     rc = qcd.lib().qcd_cg_solve(C.c_void_p(x.data_ptr()), C.c_void_p(b.data_ptr()), 1e-8, 500)
     assert rc == qcd.EINVAL
+
+
+@pytest.mark.parametrize("dims", [(6, 6, 2, 4), (10, 6, 4, 2), (2, 2, 2, 2)])
+@pytest.mark.parametrize("mode", [2, 0, 1])
+@pytest.mark.parametrize("mixed", [False, True])
+def test_cg_fused_iteration_on_ragged_lattices(dims, mode, mixed):
+    """Vh = 144, 240, 8: not multiples of the 64-thread hop block, so the launches that carry the fused
+    |t|^2 and the fused residual update run with inactive threads in their last block (they compute a
+    clamped site, store nothing and add nothing to the norm).  Against the oracle, all three forms."""
+    c = ctx()
+    kappa, csw, tol = 0.125, 1.0, 1e-10
+    U, g_hi, c_hi, A, Ainv = setup_operator(c, dims, kappa, csw, 8, 18)
+    g_lo = c.gauge_load(to_dev(U, 8), dims, 4, 12, -1) if mixed else None
+    c_lo = c.clover_build(g_hi, kappa, csw, 4) if mixed else None
+    b = inputs.spinor_field(dims, 0, 1)
+    if mode != 2:
+        b = b * (parity_mask(dims) == mode)
+    if mixed:
+        x_ref, st_ref = orc.cg_mixed(b, U, dims, kappa, tol, 5000, A, Ainv, -1, mode, 0.1)
+    else:
+        x_ref, st_ref = orc.cg(b, U, dims, kappa, tol, 5000, A, Ainv, -1, mode)
+    c.set_workspace(None)
+    c.ensure_workspace(max(c.workspace_bytes(dims, 8), 1 << 16))
+    c.set_operator(g_hi, g_lo, c_hi, c_lo, kappa, csw, mode, 0.1)
+    pb = pack(c, b, dims, 8)
+    if mode == 2:
+        x = torch.empty_like(pb)
+        rc, st = c.cg_solve(x, pb, tol, 5000)
+        got = unpack(c, x, dims)
+    else:
+        full = torch.zeros_like(pb)
+        rc, st = c.cg_solve(blocks(full)[mode], blocks(pb)[mode].clone(), tol, 5000)
+        got = unpack(c, full, dims)
+    assert rc == 0 and st.converged == 1
+    assert abs(st.iters - st_ref["iters"]) <= 2
+    assert st.r_true < 1.5 * tol
+    assert relerr(got, x_ref) <= 1e-8
