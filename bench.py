@@ -55,6 +55,7 @@ def parse_args():
     ap.add_argument("--config4-only", action="store_true", help="only the configs[4] section (for ncu passes)")
     ap.add_argument("--cheb-degree", type=int, default=100, help="Chebyshev degree timed in the configs[4] section")
     ap.add_argument("--table-scale", type=float, default=1.0, help="scale the iteration counts of the kernel table")
+    ap.add_argument("--l2-probe", action="store_true", help="only: read rate of qcd_redot on L2-resident vectors (L2 -> SM fabric)")
     return ap.parse_args()
 
 
@@ -481,6 +482,37 @@ def config_table(c, peak, config4, only4=False, cheb_degree=100):
     return out
 
 
+def l2_probe():
+    """Read rate of a pure streaming kernel (qcd_redot, fp64) on vectors that stay resident in the 126 MB L2:
+    what the L2 -> SM fabric delivers on this part, for profiles/hop_cheb_mrhs_r2.md.  Launch overhead is in
+    the per-launch time, so the rate is read off the increments between sizes."""
+    import torch
+    from paper_2001_05706_b200 import build, qcd
+    build.build()
+    c = qcd.Context(0)
+    sampler = ClockSampler(0)
+    sampler.start()
+    rows = []
+    for mb in (16, 32, 48, 64, 80, 96, 112, 160, 1024):
+        n = mb * (1 << 20) // 16
+        x = torch.randn(n, device="cuda", dtype=torch.float64)
+        y = torch.randn(n, device="cuda", dtype=torch.float64)
+        for _ in range(50):
+            c.redot(x, y, fetch=False)
+        torch.cuda.synchronize()
+        best = 1e9
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(1000):
+                c.redot(x, y, fetch=False)
+            e1.record(); e1.synchronize()
+            best = min(best, e0.elapsed_time(e1))          # us per launch (1000 launches, ms total)
+        rows.append({"MB": mb, "us_per_launch": round(best, 2), "TB/s_incl_launch": round(mb * 1.048576 / best, 2)})
+        del x, y
+    print(json.dumps({"l2_probe": rows, "clocks": sampler.stop()}))
+
+
 def max_over_ranks(ms, device="cuda"):
     """Multi-GPU timing rule: every rank contributes its device time, the job's time is the MAX
     (replicas only: no data-path collective, this all-reduce is outside the timed region)."""
@@ -660,7 +692,9 @@ def replica_command(ngpus, port, argv):
 if __name__ == "__main__":
     a = parse_args()
     TABLE_SCALE = a.table_scale
-    if a.impl == "reference":
+    if a.l2_probe:
+        l2_probe()
+    elif a.impl == "reference":
         run_reference(a)
     elif a.gpus > 1 and "WORLD_SIZE" not in os.environ:
         spawn_replicas(a)

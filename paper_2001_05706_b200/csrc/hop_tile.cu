@@ -7,8 +7,8 @@
  *
  * Why.  ncu on the round-1 kernel (one thread per site, 128 consecutive sites per block, every
  * neighbour read through L1/L2; profiles/hop_cheb_mrhs_r2.md): 897 B per site-vector cross the
- * L2 -> SM fabric for 512 B of algorithmic traffic, 9.6 TB/s at 1.59 GHz -- the fabric, not HBM,
- * is what the kernel saturates.  Each input spinor is wanted by 8 output sites; when a block
+ * L2 -> SM fabric for 512 B of algorithmic traffic, 9.6 TB/s at 1.59 GHz, and the kernel's time follows
+ * those bytes (HBM is at 74 %).  Each input spinor is wanted by 8 output sites; when a block
  * owns a compact 4-D tile most of those sites are its own, so it fetches the tile's rows once
  * per vector into shared memory (cp.async, 16 B per request, no registers) and the neighbour
  * reads that fall inside the tile become conflict-free LDS.128 with immediate offsets.
