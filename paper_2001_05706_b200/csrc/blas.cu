@@ -15,6 +15,16 @@ constexpr int BLAS_THREADS = 256;
 #define BLAS_UNROLL 4 /* grid-stride loops unrolled: cg_update fp32 0.88 -> 0.94, fp64 0.91 -> 0.96 of the roofline (1 / 2 / 4 swept) */
 #endif
 constexpr int BLAS_UNROLL_N = BLAS_UNROLL;
+/* The reductions take BLAS_BATCH grid strides at a time and issue all their loads before the first use: a
+ * `#pragma unroll` of a grid-stride loop keeps its early-exit test between the copies, and ptxas then leaves
+ * one load in flight per thread (SASS of round 1's dot_kernel: LDG, 4 x F2F + DFMA, BRA, LDG, ...).  Measured on
+ * B200 (100 MB vectors, rotating operands): norm2 fp32 22.0 -> 20.5 us, fp64 36.5 -> 34.4 us; the same change in
+ * axpby / cg_update / cg_xp moved nothing (they have 3 - 6 streams in flight per iteration anyway) and was not kept.
+ * What is left of a short reduction is fixed cost: 6.3 us per launch at 16 MB (`bench.py --l2-probe`). */
+#ifndef BLAS_BATCH
+#define BLAS_BATCH 2 /* 2 / 4 / 8 swept: norm2 the same; redot fp32 34.9 / 37.4 / 34.8 us (4 costs it two resident blocks) */
+#endif
+constexpr int BLAS_BATCH_N = BLAS_BATCH;
 
 __device__ __forceinline__ double eval(const DevScalar& s)
 {
@@ -92,8 +102,25 @@ __global__ void __launch_bounds__(BLAS_THREADS) dot_kernel(const T* __restrict__
     const V* xv = reinterpret_cast<const V*>(x);
     const V* yv = reinterpret_cast<const V*>(y);
     double s = 0.0;
-#pragma unroll BLAS_UNROLL_N
-    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
+    const size_t stride = (size_t)gridDim.x * BLAS_THREADS;
+    size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x;
+    for (; i + (BLAS_BATCH_N - 1) * stride < nvec; i += BLAS_BATCH_N * stride) {
+        V xb[BLAS_BATCH_N], yb[BLAS_BATCH_N];
+#pragma unroll
+        for (int u = 0; u < BLAS_BATCH_N; u++) {
+            xb[u] = xv[i + u * stride];
+            if (TWO) yb[u] = yv[i + u * stride];
+        }
+#pragma unroll
+        for (int u = 0; u < BLAS_BATCH_N; u++) {
+            T xs[Vec<T>::reals], ys[Vec<T>::reals];
+            vec_get(xb[u], xs);
+            if (TWO) vec_get(yb[u], ys);
+#pragma unroll
+            for (int k = 0; k < Vec<T>::reals; k++) s += (double)xs[k] * (double)(TWO ? ys[k] : xs[k]);
+        }
+    }
+    for (; i < nvec; i += stride) {
         T xs[Vec<T>::reals], ys[Vec<T>::reals];
         vec_get(xv[i], xs);
         if (TWO) vec_get(yv[i], ys);
