@@ -34,6 +34,13 @@
  *    printing.  qcd_last_error() returns text for the last error of this thread.
  *  - There is no CPU fallback anywhere: without a CUDA device every compute call
  *    returns QCD_ECUDA.
+ *  - Every entry point runs on the device of its ctx (it calls cudaSetDevice).
+ *  - Environment (read at call time, for experiments; none changes a result beyond rounding order):
+ *      QCD_CG_RUNAHEAD=n  iterations the CG drivers may enqueue ahead of the device (default 0; any n gives
+ *                         bit-identical solves, the kernels enqueued past the stopping iteration skip themselves)
+ *      QCD_MRHS_TILE=1    multi-right-hand-side hop: opt into the shared-memory tile kernel (slower on B200,
+ *                         DESIGN.md section 6); QCD_MRHS_VARIANT=40|41|31|32 picks its staging variant
+ *      QCD_TRACE=1        the mixed solver prints its reliable updates to stderr
  */
 #ifndef QCD_B200_H
 #define QCD_B200_H
