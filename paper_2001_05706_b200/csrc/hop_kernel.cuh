@@ -436,12 +436,10 @@ __global__ void __launch_bounds__(HOP_THREADS, (sizeof(T) == 4 ? HOP_MINBLOCKS_F
  * 8 x 128 links are read from HBM once, parked in per-thread shared-memory slots and reused
  * for every vector, so the link traffic per site-vector is 8*RECON reals / nvec.  out may alias
  * tm (same index, same thread). */
-template <typename T, typename Links>
-__device__ __forceinline__ void cheb_vector(const HopArgs<T>& A, const Links& L, size_t off, size_t Vh, int cb, const Neighbours<T>& nb)
+template <typename T>
+__device__ __forceinline__ void cheb_epilogue(const HopArgs<T>& A, T (&acc)[24], size_t off, size_t Vh, int cb)
 {
-    const PlaneSpinor<T> src = {A.in + off, Vh};
-    T acc[24], zz[24];
-    hop_site<T, 0>(acc, L, src, cb, nb);
+    T zz[24];
     load_planes_cs<T, 24>(zz, A.z + off, Vh, (size_t)cb);
 #pragma unroll
     for (int i = 0; i < 24; i++) {
@@ -459,6 +457,15 @@ __device__ __forceinline__ void cheb_vector(const HopArgs<T>& A, const Links& L,
         for (int i = 0; i < 24; i++) acc[i] += A.c2 * zz[i];
     }
     store_planes_cs<T, 24>(A.out + off, Vh, (size_t)cb, acc);
+}
+
+template <typename T, typename Links>
+__device__ __forceinline__ void cheb_vector(const HopArgs<T>& A, const Links& L, size_t off, size_t Vh, int cb, const Neighbours<T>& nb)
+{
+    const PlaneSpinor<T> src = {A.in + off, Vh};
+    T acc[24];
+    hop_site<T, 0>(acc, L, src, cb, nb);
+    cheb_epilogue<T>(A, acc, off, Vh, cb);
 }
 
 #ifndef HOP_CHEB_PREFETCH
@@ -496,26 +503,50 @@ __device__ __forceinline__ void cheb_prefetch(const HopArgs<T>& A, size_t off, s
     }
 }
 
+#ifndef HOP_MRHS_MINBLOCKS_F32
+#define HOP_MRHS_MINBLOCKS_F32 4
+#endif
+/* Traversal order of the multi-rhs kernels: (x,y) fastest, then t inside a tile of tblock slices, then z,
+ * then the tiles: with nvec vectors in flight the L2 footprint between the two uses of a +-t neighbour is
+ * nvec planes instead of nvec time-slices, and between +-z uses nvec*tblock planes; only the tile faces in
+ * t are fetched twice. */
+__device__ __forceinline__ int mrhs_site(const DevGeom& g, int tblock, int cb)
+{
+    if (tblock <= 1) return cb;
+    const unsigned P = (unsigned)(g.X2 * g.Y), TB = (unsigned)tblock, Z = (unsigned)g.Z;
+    unsigned r = (unsigned)cb;
+    const unsigned xy = r % P; r /= P;
+    const unsigned tin = r % TB; r /= TB;
+    const unsigned z = r % Z; const unsigned tout = r / Z;
+    return (int)(xy + P * (z + Z * (tout * TB + tin)));
+}
+
+template <typename T, int RECON>
+__device__ __forceinline__ void park_links(const SmemLinks<T, RECON>& S, const GlobalLinks<T, RECON>& G, int cb, const Neighbours<T>& nb)
+{
+    T u[18];
+    G.template get<0, +1>(u, cb, nb.xp); S.template put<0, +1>(u);
+    G.template get<0, -1>(u, cb, nb.xm); S.template put<0, -1>(u);
+    G.template get<1, +1>(u, cb, nb.yp); S.template put<1, +1>(u);
+    G.template get<1, -1>(u, cb, nb.ym); S.template put<1, -1>(u);
+    G.template get<2, +1>(u, cb, nb.zp); S.template put<2, +1>(u);
+    G.template get<2, -1>(u, cb, nb.zm); S.template put<2, -1>(u);
+    G.template get<3, +1>(u, cb, nb.tp); S.template put<3, +1>(u);
+    G.template get<3, -1>(u, cb, nb.tm); S.template put<3, -1>(u);
+}
+
+#ifndef HOP_MRHS_MINBLOCKS_F32
+#define HOP_MRHS_MINBLOCKS_F32 4
+#endif
 /* STAGE = 1: nvec > 1, links parked in shared memory; STAGE = 0: one vector, links straight from HBM */
 template <typename T, int RECON, int STAGE>
-__global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_cheb_mrhs_kernel(const HopArgs<T> A)
+__global__ void __launch_bounds__(128, (sizeof(T) == 4 ? HOP_MRHS_MINBLOCKS_F32 : 2)) hop_cheb_mrhs_kernel(const HopArgs<T> A)
 {
     typedef typename Vec<T>::type V;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= A.geo.Vh) return;
-    if (STAGE && A.tblock > 1) {
-        /* Traversal order (x,y) fastest, then t inside a tile of tblock slices, then z, then the
-         * tiles: with nvec vectors in flight the L2 footprint between the two uses of a +-t
-         * neighbour is nvec planes instead of nvec time-slices, and between +-z uses nvec*tblock
-         * planes; only the tile faces in t are fetched twice. */
-        const unsigned P = (unsigned)(A.geo.X2 * A.geo.Y), TB = (unsigned)A.tblock, Z = (unsigned)A.geo.Z;
-        unsigned r = (unsigned)cb;
-        const unsigned xy = r % P; r /= P;
-        const unsigned tin = r % TB; r /= TB;
-        const unsigned z = r % Z; const unsigned tout = r / Z;
-        cb = (int)(xy + P * (z + Z * (tout * TB + tin)));
-    }
+    if (STAGE) cb = mrhs_site(A.geo, A.tblock, cb);
     const size_t Vh = (size_t)A.geo.Vh;
     const Neighbours<T> nb(A.geo, cb, A.parity, A.tb);
     const GlobalLinks<T, RECON> G = {A.gauge, A.gblock, Vh, A.parity};
@@ -525,17 +556,7 @@ __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? 4 : 2)) hop_cheb_mrhs_k
     }
     const SmemLinks<T, RECON> S = {reinterpret_cast<V*>(smem_raw) + threadIdx.x};
     if (HOP_CHEB_PREFETCH & 4) cheb_prefetch<T, 1>(A, 0, Vh, cb, nb);
-    {
-        T u[18];
-        G.template get<0, +1>(u, cb, nb.xp); S.template put<0, +1>(u);
-        G.template get<0, -1>(u, cb, nb.xm); S.template put<0, -1>(u);
-        G.template get<1, +1>(u, cb, nb.yp); S.template put<1, +1>(u);
-        G.template get<1, -1>(u, cb, nb.ym); S.template put<1, -1>(u);
-        G.template get<2, +1>(u, cb, nb.zp); S.template put<2, +1>(u);
-        G.template get<2, -1>(u, cb, nb.zm); S.template put<2, -1>(u);
-        G.template get<3, +1>(u, cb, nb.tp); S.template put<3, +1>(u);
-        G.template get<3, -1>(u, cb, nb.tm); S.template put<3, -1>(u);
-    }
+    park_links<T, RECON>(S, G, cb, nb);
     for (int j = 0; j < A.nvec; j++) {
         /* bit 0: own-site streams of this vector now; bit 2: of the next vector instead;
          * bit 1: x neighbours of the next vector; bit 3: all its neighbours */
