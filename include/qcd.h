@@ -119,6 +119,9 @@ int qcd_clover_free(qcd_clover* c);
 /* Debug / parity: expand A (which=0) or A^-1 (which=1) to boundary-order dense
  * [t][z][y][x][12][12][re,im] fp64 (DEVICE, V*288 doubles). */
 int qcd_clover_unpack(qcd_ctx* ctx, void* dense, const qcd_clover* c, int which);
+/* out = A in (inverse = 0) or A^-1 in (inverse = 1) on the sites of one parity (SURVEY 8(a) a7 as a
+ * stand-alone, site-local step): in/out one-parity blocks in the handle's precision (4|8), out == in allowed. */
+int qcd_clover_apply(qcd_ctx* ctx, void* out, const void* in, const qcd_clover* c, int inverse, int parity);
 
 /* ---- spinor layout conversion (boundary <-> internal, both DEVICE) ---------------- */
 size_t qcd_spinor_bytes(const int dims[4], int precision);   /* full lattice */
@@ -226,6 +229,18 @@ int qcd_cg_multishift(qcd_ctx* ctx, void* x, const void* b, const double* shifts
 /* out = M in (flags & QCD_DAGGER: M^dag in) for the operator of qcd_set_operator, in
  * the high precision. */
 int qcd_apply_operator(qcd_ctx* ctx, void* out, const void* in, int flags);
+/* Even-odd source preparation and solution reconstruction (SURVEY.md 8(c) reading O5; the even-odd
+ * preconditioning is north_star's, PAPER.md names only the "inverter" that uses it) for the
+ * operator of qcd_set_operator with parity p = 0|1, pb = 1 - p, in its high precision:
+ *   qcd_eo_prepare:      bhat_p = b_p + kappa H_{p,pb} A^-1_{pb} b_pb
+ *   qcd_eo_reconstruct:  x_pb   = A^-1_{pb} (b_pb + kappa H_{pb,p} x_p)
+ * so that Mhat x_p = bhat_p (e.g. x_p from qcd_cg_solve on Mhat^dag bhat_p) followed by the reconstruction
+ * solves the full system (A - kappa H) x = b.  b: full field (even block, then odd block), read only;
+ * bhat: one-parity block, must not overlap b; x: full field whose parity-p block is read and whose
+ * parity-pb block is written, must not overlap b.  With a clover term qcd_eo_prepare uses one parity
+ * block of the workspace (qcd_set_workspace) as scratch.  QCD_EINVAL if no even-odd operator is set. */
+int qcd_eo_prepare(qcd_ctx* ctx, void* bhat, const void* b);
+int qcd_eo_reconstruct(qcd_ctx* ctx, void* x, const void* b);
 
 /* ---- Chebyshev driver (reading O8/S16) ----
  * y = sum_{k=0}^{degree} coeff[k] T_k(H_W/scale) v,  H_W = gamma5 (1 - kappa H), full

@@ -4,6 +4,20 @@
 cudaError_t hop_launch_f32(const qcd_gauge* g, const HopLaunch& L, cudaStream_t st);
 cudaError_t hop_launch_f64(const qcd_gauge* g, const HopLaunch& L, cudaStream_t st);
 
+cudaError_t clover_site_launch_f32(void* out, const void* in, const void* clov, int Vh, cudaStream_t st);
+cudaError_t clover_site_launch_f64(void* out, const void* in, const void* clov, int Vh, cudaStream_t st);
+
+/* out = C in on one parity; block = 0,1: A of parity 0,1; 2,3: A^-1 of parity 0,1 */
+int clover_site_apply(qcd_ctx* ctx, void* out, const void* in, const qcd_clover* c, int block)
+{
+    const void* clov = (const char*)c->data + (size_t)block * c->block_bytes;
+    const cudaError_t e = (c->precision == 4) ? clover_site_launch_f32(out, in, clov, c->geo.Vh, ctx->stream)
+                                              : clover_site_launch_f64(out, in, clov, c->geo.Vh, ctx->stream);
+    if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "clover apply launch: %s", cudaGetErrorString(e));
+    ctx->launches++;
+    return QCD_OK;
+}
+
 int hop_norm_scratch(qcd_ctx* ctx, size_t nblocks)
 {
     if (ctx->hop_partial_cap >= nblocks) return QCD_OK;

@@ -13,3 +13,8 @@ cudaError_t hop_launch_f32(const qcd_gauge* g, const HopLaunch& L, cudaStream_t 
     HopArgs<float> A = make_hop_args<float>(g, L);
     return hop_dispatch<float>(A, g->reconstruct, L.dagger, L.mode, st);
 }
+
+cudaError_t clover_site_launch_f32(void* out, const void* in, const void* clov, int Vh, cudaStream_t st)
+{
+    return clover_site_launch<float>(out, in, clov, Vh, st);
+}

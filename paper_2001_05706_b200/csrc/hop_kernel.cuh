@@ -597,6 +597,25 @@ template <typename T, int RECON, int DAG> static cudaError_t hop_dispatch_mode(c
     return cudaGetLastError();
 }
 
+/* out(cb) = C(cb) in(cb) on one parity, C = A or A^-1 (two packed Hermitian 6x6 blocks per site).
+ * Site-local, so out may be in.  Used by the even-odd source preparation / solution reconstruction (reading O5). */
+template <typename T>
+__global__ void __launch_bounds__(128) clover_site_kernel(T* out, const T* in, const T* __restrict__ clov, int Vh)
+{
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= Vh) return;
+    T v[24], o[24];
+    load_planes_rw<T, 24>(v, in, (size_t)Vh, (size_t)cb);
+    clover_apply<T>(o, clov, (size_t)Vh, (size_t)cb, v);
+    store_planes<T, 24>(out, (size_t)Vh, (size_t)cb, o);
+}
+
+template <typename T> static cudaError_t clover_site_launch(void* out, const void* in, const void* clov, int Vh, cudaStream_t st)
+{
+    clover_site_kernel<T><<<(Vh + 127) / 128, 128, 0, st>>>((T*)out, (const T*)in, (const T*)clov, Vh);
+    return cudaGetLastError();
+}
+
 template <typename T> static cudaError_t hop_dispatch(const HopArgs<T>& A, int recon, int dagger, int mode, cudaStream_t st)
 {
     if (mode == HOP_CHEB) return recon == 12 ? hop_cheb_launch<T, 12>(A, st) : hop_cheb_launch<T, 18>(A, st);

@@ -148,6 +148,7 @@ struct HopLaunch {
 };
 
 int hop_launch(qcd_ctx* ctx, const qcd_gauge* g, const HopLaunch& L);
+int clover_site_apply(qcd_ctx* ctx, void* out, const void* in, const qcd_clover* c, int block); /* hop.cu: block 0,1 = A, 2,3 = A^-1 */
 enum { HOP_NORM_GROUP = 64 }; /* blocks per first-level group of the fused norm's reduction */
 int hop_norm_scratch(qcd_ctx* ctx, size_t nblocks); /* hop.cu: make the scratch of the fused norm hold nblocks blocks */
 void solver_forget_ctx(const qcd_ctx* ctx); /* solver.cu: qcd_finalize clears the "last ctx" of qcd_cg_solve */

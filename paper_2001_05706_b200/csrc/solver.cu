@@ -358,6 +358,64 @@ int qcd_apply_operator(qcd_ctx* ctx, void* out, const void* in, int flags)
     return qcd_dslash_ex(out, in, ctx->g_hi, ctx->c_hi, ctx->kappa, ctx->csw, ctx->op_parity, flags, nullptr);
 }
 
+/* Even-odd source preparation and solution reconstruction (reading O5) in the high precision of the
+ * operator of qcd_set_operator; p = its parity, pb = 1 - p; full fields hold the even block, then the odd one. */
+static inline size_t eo_block_bytes(const qcd_ctx* ctx) { return (size_t)ctx->g_hi->geo.Vh * 24 * ctx->g_hi->precision; }
+
+int qcd_eo_prepare(qcd_ctx* ctx, void* bhat, const void* b)
+{
+    QCD_REQUIRE(ctx && ctx->op_set, "eo_prepare: no operator set (qcd_set_operator)");
+    QCD_REQUIRE(ctx->op_parity == 0 || ctx->op_parity == 1, "eo_prepare: the operator set is the full-lattice one");
+    QCD_REQUIRE(bhat && b && (((uintptr_t)bhat | (uintptr_t)b) & 15u) == 0, "eo_prepare: pointers must be non-NULL, 16-byte aligned");
+    const size_t blk = eo_block_bytes(ctx);
+    const char* bc = (const char*)b;
+    QCD_REQUIRE((const char*)bhat + blk <= bc || bc + 2 * blk <= (const char*)bhat, "eo_prepare: bhat and b alias");
+    QCD_ON_DEVICE(ctx);
+    const int p = ctx->op_parity, pb = 1 - p;
+    const void* t = bc + (size_t)pb * blk;
+    if (ctx->c_hi) { /* t = Ainv_pb b_pb */
+        QCD_REQUIRE(ctx->ws && ctx->ws_bytes >= blk, "eo_prepare: workspace missing (qcd_set_workspace)");
+        QCD_REQUIRE((const char*)ctx->ws + blk <= (const char*)bhat || (const char*)bhat + blk <= (const char*)ctx->ws, "eo_prepare: bhat lies in the workspace");
+        RC(clover_site_apply(ctx, ctx->ws, t, ctx->c_hi, 2 + pb));
+        t = ctx->ws;
+    }
+    HopLaunch L;
+    memset(&L, 0, sizeof(L));
+    L.out = bhat; L.in = t; L.z = bc + (size_t)p * blk; L.a = 1.0; L.b = ctx->kappa; L.out_parity = p; L.mode = HOP_XPAY;
+    return hop_launch(ctx, ctx->g_hi, L);
+}
+
+int qcd_eo_reconstruct(qcd_ctx* ctx, void* x, const void* b)
+{
+    QCD_REQUIRE(ctx && ctx->op_set, "eo_reconstruct: no operator set (qcd_set_operator)");
+    QCD_REQUIRE(ctx->op_parity == 0 || ctx->op_parity == 1, "eo_reconstruct: the operator set is the full-lattice one");
+    QCD_REQUIRE(x && b && (((uintptr_t)x | (uintptr_t)b) & 15u) == 0, "eo_reconstruct: pointers must be non-NULL, 16-byte aligned");
+    const size_t blk = eo_block_bytes(ctx);
+    QCD_REQUIRE((char*)x + 2 * blk <= (const char*)b || (const char*)b + 2 * blk <= (char*)x, "eo_reconstruct: x and b alias");
+    QCD_ON_DEVICE(ctx);
+    const int p = ctx->op_parity, pb = 1 - p;
+    char* x_pb = (char*)x + (size_t)pb * blk;
+    HopLaunch L;
+    memset(&L, 0, sizeof(L)); /* x_pb = b_pb + kappa H_{pb,p} x_p */
+    L.out = x_pb; L.in = (char*)x + (size_t)p * blk; L.z = (const char*)b + (size_t)pb * blk; L.a = 1.0; L.b = ctx->kappa;
+    L.out_parity = pb; L.mode = HOP_XPAY;
+    RC(hop_launch(ctx, ctx->g_hi, L));
+    if (ctx->c_hi) RC(clover_site_apply(ctx, x_pb, x_pb, ctx->c_hi, 2 + pb)); /* site-local: in place */
+    return QCD_OK;
+}
+
+int qcd_clover_apply(qcd_ctx* ctx, void* out, const void* in, const qcd_clover* c, int inverse, int parity)
+{
+    QCD_REQUIRE(ctx && c && c->ctx == ctx, "clover_apply: NULL handle or clover of another context");
+    QCD_REQUIRE(c->precision == 4 || c->precision == 8, "clover_apply: needs an fp32 or fp64 clover handle");
+    QCD_REQUIRE(parity == 0 || parity == 1, "clover_apply: parity must be 0|1");
+    QCD_REQUIRE(out && in && (((uintptr_t)out | (uintptr_t)in) & 15u) == 0, "clover_apply: pointers must be non-NULL, 16-byte aligned");
+    const size_t blk = (size_t)c->geo.Vh * 24 * c->precision;
+    QCD_REQUIRE(out == in || (char*)out + blk <= (const char*)in || (const char*)in + blk <= (char*)out, "clover_apply: out and in overlap partially");
+    QCD_ON_DEVICE(ctx);
+    return clover_site_apply(ctx, out, in, c, (inverse ? 2 : 0) + parity);
+}
+
 int qcd_cg_solve_ex(qcd_ctx* ctx, void* x, const void* b, double tol, int maxiter, qcd_stats* stats)
 {
     QCD_REQUIRE(ctx && ctx->op_set, "cg_solve: no operator set (qcd_set_operator)");

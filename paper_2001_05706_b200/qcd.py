@@ -78,6 +78,9 @@ SIGNATURES = {
     "qcd_cg_solve_ex": (_i, [_vp, _vp, _vp, _d, _i, C.POINTER(Stats)]),
     "qcd_cg_multishift": (_i, [_vp, _vp, _vp, C.POINTER(_d), _i, _d, _i, C.POINTER(Stats), C.POINTER(_d)]),
     "qcd_apply_operator": (_i, [_vp, _vp, _vp, _i]),
+    "qcd_eo_prepare": (_i, [_vp, _vp, _vp]),
+    "qcd_eo_reconstruct": (_i, [_vp, _vp, _vp]),
+    "qcd_clover_apply": (_i, [_vp, _vp, _vp, _vp, _i, _i]),
     "qcd_cheb_apply": (_i, [_vp, _vp, _vp, _vp, _d, C.POINTER(_d), _i, _d]),
     "qcd_cheb_apply_multi": (_i, [_vp, _vp, _vp, _i, _vp, _d, C.POINTER(_d), _i, _d]),
     "qcd_hop_host": (_i, [_vp, _vp, _vp, _vp, _i, _i]),
@@ -295,6 +298,15 @@ class Context:
 
     def apply_operator(self, out, inp, flags: int = 0):
         _check(lib().qcd_apply_operator(self.h, _ptr(out), _ptr(inp), flags))
+
+    def eo_prepare(self, bhat, b):
+        _check(lib().qcd_eo_prepare(self.h, _ptr(bhat), _ptr(b)))
+
+    def eo_reconstruct(self, x, b):
+        _check(lib().qcd_eo_reconstruct(self.h, _ptr(x), _ptr(b)))
+
+    def clover_apply(self, out, inp, clover, inverse: bool, parity: int):
+        _check(lib().qcd_clover_apply(self.h, _ptr(out), _ptr(inp), clover.h, int(bool(inverse)), parity))
 
     def cg_solve(self, x, b, tol: float, maxiter: int):
         """Returns (return code, Stats). QCD_NOCONV (1) is returned, not raised."""

@@ -6,7 +6,7 @@ import pytest
 import torch
 
 from oracle import oracle as orc
-from paper_2001_05706_b200 import inputs
+from paper_2001_05706_b200 import inputs, qcd
 
 from gpu_util import TOL, blocks, ctx, pack, parity_mask, relerr, to_dev, unpack
 
@@ -465,3 +465,103 @@ def test_cg_fused_iteration_on_ragged_lattices(dims, mode, mixed):
     assert abs(st.iters - st_ref["iters"]) <= 2
     assert st.r_true < 1.5 * tol
     assert relerr(got, x_ref) <= 1e-8
+
+
+@pytest.mark.parametrize("dims", [(8, 8, 8, 16), (6, 4, 2, 8)])
+@pytest.mark.parametrize("p", [0, 1])
+@pytest.mark.parametrize("csw,precision,recon", [(0.0, 8, 18), (1.0, 8, 18), (1.0, 8, 12), (1.0, 4, 12)])
+def test_even_odd_source_preparation_and_reconstruction_match_oracle(dims, p, csw, precision, recon):
+    """Reading O5, second half: bhat_p = b_p + kappa H A^-1 b_pb and x_pb = A^-1 (b_pb + kappa H x_p),
+    each against the oracle's definition on the same inputs (x_p a random field, not a solution)."""
+    c = ctx()
+    kappa = 0.135
+    U, g, cl, A, Ainv = setup_operator(c, dims, kappa, csw, precision, recon)
+    b = inputs.spinor_field(dims, 3, 1)
+    xp = inputs.spinor_field(dims, 4, 1) * (parity_mask(dims) == p)
+    if precision == 4:
+        b, xp = inputs.round_to_f32(b), inputs.round_to_f32(xp)
+    want_bhat = orc.eo_prepare_source(b, U, dims, kappa, Ainv, -1, p)
+    want_x = orc.eo_reconstruct(xp, b, U, dims, kappa, Ainv, -1, p)
+    c.ensure_workspace(c.workspace_bytes(dims, precision))
+    c.set_operator(g, None, cl, None, kappa, csw, p)
+    pb = pack(c, b, dims, precision)
+    before = pb.clone()
+    full = torch.zeros_like(pb)
+    c.eo_prepare(blocks(full)[p], pb)
+    assert relerr(unpack(c, full, dims), want_bhat) <= TOL[precision]
+    assert torch.equal(blocks(full)[1 - p], torch.zeros_like(blocks(full)[1 - p]))   # only the parity-p block is written
+    x = pack(c, xp, dims, precision)
+    x_p_before = blocks(x)[p].clone()
+    c.eo_reconstruct(x, pb)
+    assert torch.equal(blocks(x)[p], x_p_before)
+    assert relerr(unpack(c, x, dims), want_x) <= TOL[precision]
+    assert torch.equal(pb, before)
+
+
+@pytest.mark.parametrize("csw", [0.0, 1.0])
+def test_full_system_solved_through_the_even_odd_operator(csw):
+    """P8 on the GPU: prepare, CG on Mhat^dag Mhat, reconstruct; the result solves (A - kappa H) x = b,
+    agrees with the oracle doing the same, and takes the oracle's iteration count +-2."""
+    c = ctx()
+    dims, kappa, tol = (8, 8, 8, 16), 0.135, 1e-11
+    U, g, cl, A, Ainv = setup_operator(c, dims, kappa, csw, 8, 18)
+    b = inputs.spinor_field(dims, 10, 1)
+    bhat = orc.eo_prepare_source(b, U, dims, kappa, Ainv)
+    rhs = orc.apply_M(bhat, U, dims, kappa, A, Ainv, mode=0, dagger=True)
+    xe, st_ref = orc.cg(rhs, U, dims, kappa, tol, 5000, A, Ainv, -1, 0)
+    x_ref = orc.eo_reconstruct(xe, b, U, dims, kappa, Ainv)
+
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    c.set_operator(g, None, cl, None, kappa, csw, 0)
+    pb = pack(c, b, dims, 8)
+    half = blocks(pb)[0].numel()
+    bh = torch.empty(half, dtype=pb.dtype, device="cuda")
+    rh = torch.empty_like(bh)
+    c.eo_prepare(bh, pb)
+    c.apply_operator(rh, bh, qcd.DAGGER)
+    x = torch.zeros_like(pb)
+    rc, st = c.cg_solve(blocks(x)[0], rh, tol, 5000)
+    assert rc == 0 and abs(st.iters - st_ref["iters"]) <= 2
+    c.eo_reconstruct(x, pb)
+    got = unpack(c, x, dims)
+    assert relerr(got, x_ref) <= 1e-9
+    Dx = torch.empty_like(pb)
+    c.dslash(Dx, x, g, cl, kappa, csw, 2)
+    assert relerr(unpack(c, Dx, dims), b) <= 1e-9
+
+
+@pytest.mark.parametrize("precision", [8, 4])
+@pytest.mark.parametrize("inverse", [False, True])
+def test_clover_apply_matches_oracle_and_works_in_place(precision, inverse):
+    c = ctx()
+    dims, kappa, csw = (6, 4, 2, 8), 0.135, 1.0
+    U, g, cl, A, Ainv = setup_operator(c, dims, kappa, csw, precision, 18)
+    v = inputs.spinor_field(dims, 5, 1)
+    if precision == 4:
+        v = inputs.round_to_f32(v)
+    pv = pack(c, v, dims, precision)
+    out = torch.zeros_like(pv)
+    for p in (0, 1):
+        c.clover_apply(blocks(out)[p], blocks(pv)[p], cl, inverse, p)
+    want = sum(orc.site_matrix_apply(Ainv if inverse else A, v * (parity_mask(dims) == p), dims, p) for p in (0, 1))
+    assert relerr(unpack(c, out, dims), want) <= TOL[precision]
+    for p in (0, 1):
+        c.clover_apply(blocks(pv)[p], blocks(pv)[p], cl, inverse, p)
+    assert torch.equal(pv, out)
+
+
+def test_even_odd_helpers_argument_errors():
+    c = ctx()
+    dims, kappa = (4, 4, 4, 4), 0.135
+    U, g, cl, A, Ainv = setup_operator(c, dims, kappa, 0.0, 8, 18)
+    c.ensure_workspace(c.workspace_bytes(dims, 8))
+    pb = pack(c, inputs.spinor_field(dims, 0, 1), dims, 8)
+    x = torch.zeros_like(pb)
+    c.set_operator(g, None, None, None, kappa, 0.0, 2)
+    with pytest.raises(qcd.QcdError):
+        c.eo_prepare(blocks(x)[0], pb)          # full-lattice operator set
+    c.set_operator(g, None, None, None, kappa, 0.0, 0)
+    with pytest.raises(qcd.QcdError):
+        c.eo_prepare(blocks(pb)[0], pb)         # bhat inside b
+    with pytest.raises(qcd.QcdError):
+        c.eo_reconstruct(pb, pb)                # x is b
