@@ -167,6 +167,35 @@ def test_hop_whole_field_32x64(world, dagger):
         del out, got
 
 
+@pytest.mark.parametrize("clover", [False, True])
+def test_even_odd_source_preparation_and_reconstruction_whole_field_32x64(world, clover):
+    """Reading O5's two ends of an even-odd solve at full size, every site against the oracle's definitions."""
+    if clover and _host_mem_gb() < 40:
+        pytest.skip("needs ~30 GB of host memory for the oracle's dense clover fields")
+    c, U, psi, g, g18, cl, pin = world
+    h = pin.numel() // 2
+    Ainv = None
+    if clover:
+        Ainv = inputs.round_to_f32(orc.invert_12(orc.clover_matrix(orc.field_strength(U, DIMS), DIMS, KAPPA * CSW)))
+    par = orc.parity_mask_array(DIMS)[..., None, None, None]
+    c.ensure_workspace(c.workspace_bytes(DIMS, 4))
+    c.set_operator(g, None, cl if clover else None, None, KAPPA, CSW if clover else 0.0, 0)
+    out = torch.zeros_like(pin)
+    c.eo_prepare(out[:h], pin)
+    got = c.spinor_unpack(out, DIMS).cpu().numpy().astype(np.float64)
+    want = orc.eo_prepare_source(psi, U, DIMS, KAPPA, Ainv)
+    assert relerr(got, want) <= 2e-6
+    assert_every_site_close(got, want, (par == 0).ravel())
+    # reconstruction from the even block of psi standing in for a solution, b = the prepared field's source
+    x = pin.clone()
+    x[h:] = 0
+    c.eo_reconstruct(x, pin)
+    got = c.spinor_unpack(x, DIMS).cpu().numpy().astype(np.float64)
+    want = orc.eo_reconstruct(psi * (par == 0), psi, U, DIMS, KAPPA, Ainv)
+    assert relerr(got, want) <= 2e-6
+    assert_every_site_close(got, want)
+
+
 def test_operator_adjoint_identity_32x64(world):
     """Re<chi, Mhat psi> = Re<Mhat^dag chi, psi> on the full-size even block (any size property)."""
     c, U, psi, g, g18, cl, pin = world
