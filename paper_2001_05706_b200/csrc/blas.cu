@@ -69,8 +69,20 @@ __device__ __forceinline__ bool grid_sum(double v, double* partial, unsigned int
     __syncthreads();
     if (!last) return false;
     __threadfence();
+    /* the partials of up to GRID_SUM_BATCH * BLAS_THREADS blocks are requested together (L2 loads, the other blocks'
+     * stores are visible after the fence) and summed in index order: a `volatile` loop paid one L2 round trip per
+     * 256 blocks on the launch's critical path */
+    constexpr int GRID_SUM_BATCH = 8;
+    double pv[GRID_SUM_BATCH];
+#pragma unroll
+    for (int u = 0; u < GRID_SUM_BATCH; u++) {
+        const unsigned int i = threadIdx.x + u * BLAS_THREADS;
+        pv[u] = (i < gridDim.x) ? __ldcg(partial + i) : 0.0;
+    }
     double s = 0.0;
-    for (unsigned int i = threadIdx.x; i < gridDim.x; i += BLAS_THREADS) s += ((volatile double*)partial)[i];
+#pragma unroll
+    for (int u = 0; u < GRID_SUM_BATCH; u++) s += pv[u];
+    for (unsigned int i = threadIdx.x + GRID_SUM_BATCH * BLAS_THREADS; i < gridDim.x; i += BLAS_THREADS) s += __ldcg(partial + i);
     const double r = block_sum(s);
     if (threadIdx.x == 0) *tot = r;
     return threadIdx.x == 0;
