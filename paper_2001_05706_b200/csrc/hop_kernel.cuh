@@ -521,8 +521,8 @@ __device__ __forceinline__ int mrhs_site(const DevGeom& g, int tblock, int cb)
     return (int)(xy + P * (z + Z * (tout * TB + tin)));
 }
 
-template <typename T, int RECON>
-__device__ __forceinline__ void park_links(const SmemLinks<T, RECON>& S, const GlobalLinks<T, RECON>& G, int cb, const Neighbours<T>& nb)
+template <typename T, int RECON, typename Slots>
+__device__ __forceinline__ void park_links(const Slots& S, const GlobalLinks<T, RECON>& G, int cb, const Neighbours<T>& nb)
 {
     T u[18];
     G.template get<0, +1>(u, cb, nb.xp); S.template put<0, +1>(u);
@@ -556,7 +556,7 @@ __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? HOP_MRHS_MINBLOCKS_F32 
     }
     const SmemLinks<T, RECON> S = {reinterpret_cast<V*>(smem_raw) + threadIdx.x};
     if (HOP_CHEB_PREFETCH & 4) cheb_prefetch<T, 1>(A, 0, Vh, cb, nb);
-    park_links<T, RECON>(S, G, cb, nb);
+    park_links<T, RECON, SmemLinks<T, RECON> >(S, G, cb, nb);
     for (int j = 0; j < A.nvec; j++) {
         /* bit 0: own-site streams of this vector now; bit 2: of the next vector instead;
          * bit 1: x neighbours of the next vector; bit 3: all its neighbours */
