@@ -8,6 +8,12 @@
 
 #include "qcd_internal.h"
 
+/* programmatic dependent launch (sm_90+): griddepcontrol.launch_dependents lets the next launch of the stream start
+ * placing blocks once every block of this grid has executed it; griddepcontrol.wait blocks until the previous grid has
+ * completed and its memory operations are visible.  Both are no-ops in a launch without the attribute. */
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 template <typename T> struct Vec;
 template <> struct Vec<float> {
     typedef float4 type;
