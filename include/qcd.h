@@ -203,6 +203,25 @@ int qcd_redot(qcd_ctx*, const void* x, const void* y, size_t nreal, int precisio
 int qcd_cg_update(qcd_ctx*, double a, const void* p, const void* q, void* x, void* r,
                   size_t nreal, int precision, double* result);
 
+/* ---- reduction without any allocation (variant of qcd_norm2) ----
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops): needs no qcd_ctx
+ * (qcd_init allocates) and calls no cudaMalloc / cudaFree / allocating routine.  Its scratch, one fp64 partial per
+ * block of 16 KiB of x and a ticket, is a static 512 KiB + 256 B device array inside the library, which every GPU
+ * that loads the library holds until the process exits.
+ *   qcd_noalloc_setup(device)   once per device, outside any capture: takes the device address of that array
+ *                               (cudaGetSymbolAddress with `device` current).  QCD_ECUDA / QCD_EINVAL on failure.
+ *   qcd_norm2_noalloc(...)      *result_dev = sum_i x_i^2, products and sums in fp64, deterministic (the value
+ *                               depends on nreal only).  x: DEVICE, 16-byte aligned, nreal reals of `precision`
+ *                               4|8, nreal a multiple of 16/precision; result_dev: DEVICE double, written on
+ *                               cuda_stream (nothing is synchronised or copied to the host).
+ * Limit: x of at most qcd_noalloc_max_bytes() = 1 GiB (2^28 fp32 or 2^27 fp64 reals); a larger nreal is rejected
+ * with QCD_EINVAL before anything is enqueued (use qcd_norm2).  All calls on a device share the array: calls that
+ * overlap on the GPU (two streams, concurrent graph replays) race on it and must be serialised by the caller;
+ * calls on one stream are safe, the ticket is cleared on the stream before each launch. */
+size_t qcd_noalloc_max_bytes(void);
+int qcd_noalloc_setup(int device);
+int qcd_norm2_noalloc(int device, void* cuda_stream, const void* x, size_t nreal, int precision, double* result_dev);
+
 /* ---- solvers (readings O6, O7, S13, S15) ----------------------
  * qcd_set_operator selects M for the solvers of this ctx:
  *   parity 2: M = A - kappa H on the full lattice; 0|1: even-odd Schur operator.

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libqcd_b200.so")
-UNITS = ["api", "solver", "hop", "hop_f32", "hop_f64", "hop_tile", "hop_half", "blas", "layout", "clover"]
+UNITS = ["api", "solver", "hop", "hop_f32", "hop_f64", "hop_tile", "hop_half", "blas", "layout", "clover", "noalloc"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr",

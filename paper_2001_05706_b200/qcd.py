@@ -78,6 +78,9 @@ SIGNATURES = {
     "qcd_cg_solve_ex": (_i, [_vp, _vp, _vp, _d, _i, C.POINTER(Stats)]),
     "qcd_cg_multishift": (_i, [_vp, _vp, _vp, C.POINTER(_d), _i, _d, _i, C.POINTER(Stats), C.POINTER(_d)]),
     "qcd_apply_operator": (_i, [_vp, _vp, _vp, _i]),
+    "qcd_noalloc_max_bytes": (_sz, []),
+    "qcd_noalloc_setup": (_i, [_i]),
+    "qcd_norm2_noalloc": (_i, [_i, _vp, _vp, _sz, _i, _vp]),
     "qcd_eo_prepare": (_i, [_vp, _vp, _vp]),
     "qcd_eo_reconstruct": (_i, [_vp, _vp, _vp]),
     "qcd_clover_apply": (_i, [_vp, _vp, _vp, _vp, _i, _i]),
@@ -126,6 +129,20 @@ def _prec(t: torch.Tensor) -> int:
 
 def _dtype(precision: int):
     return {4: torch.float32, 8: torch.float64}[precision]
+
+
+def noalloc_max_bytes() -> int:
+    return int(lib().qcd_noalloc_max_bytes())
+
+
+def noalloc_setup(device: int = 0):
+    _check(lib().qcd_noalloc_setup(device))
+
+
+def norm2_noalloc(x: torch.Tensor, result_dev: torch.Tensor, nreal=None, device: int = 0, stream=None):
+    """result_dev[0] = |x|^2 on `stream` (default: torch's current stream); no ctx, nothing allocated."""
+    st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+    _check(lib().qcd_norm2_noalloc(device, C.c_void_p(st), _ptr(x), x.numel() if nreal is None else int(nreal), _prec(x), _ptr(result_dev)))
 
 
 def _dims(dims):

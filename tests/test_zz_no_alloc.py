@@ -1,0 +1,72 @@
+"""qcd_norm2_noalloc (include/qcd.h): the reduction whose scratch is a static device array, against the
+existing qcd_norm2 path, on calls in a row that share that array.  Collected last on purpose (file name)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2001_05706_b200 import qcd
+
+from gpu_util import ctx
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-13   # the tolerance tests/test_gpu_solvers.py::test_blas_matches_numpy_fp64 holds qcd_norm2 to
+
+
+def field(n, precision, seed):
+    rng = np.random.default_rng(seed)
+    return torch.from_numpy(rng.standard_normal(n).astype({4: np.float32, 8: np.float64}[precision])).cuda()
+
+
+@pytest.mark.parametrize("precision", [4, 8])
+def test_norm2_noalloc_matches_qcd_norm2_on_calls_in_a_row(precision):
+    c = ctx()
+    qcd.noalloc_setup(0)
+    out = torch.full((2,), -1.0, dtype=torch.float64, device="cuda")
+    # a large field first (1465 blocks' partials left behind), then a short ragged one, then a mid-sized one,
+    # then the first again: every call finds the previous call's partials and a used ticket in the array
+    sizes = [24 * 250000, 24 * 1000 + 4, 24 * 8 * 8 * 8 * 16, 24 * 250000]
+    xs = [field(n, precision, 100 + i) for i, n in enumerate(sizes[:3])]
+    xs.append(xs[0])
+    want = [c.norm2(x) for x in xs]
+    got = []
+    for x in xs:
+        qcd.norm2_noalloc(x, out[:1])
+        qcd.norm2_noalloc(x, out[1:])          # twice in a row on the same stream
+        torch.cuda.synchronize()
+        a, b = out.tolist()
+        assert a == b                          # deterministic, whatever the array held before
+        got.append(a)
+    for g, w, x in zip(got, want, xs):
+        assert abs(g - w) <= RTOL * w
+        x64 = x.double().cpu().numpy()
+        assert abs(g - np.dot(x64, x64)) <= RTOL * np.dot(x64, x64)
+    assert got[0] == got[3]
+
+
+def test_norm2_noalloc_allocates_nothing_and_rejects_what_the_scratch_cannot_cover():
+    qcd.noalloc_setup(0)
+    x = field(24 * 100000, 4, 7)
+    out = torch.zeros(1, dtype=torch.float64, device="cuda")
+    qcd.norm2_noalloc(x, out)                  # first launch: the kernel's code is loaded now
+    torch.cuda.synchronize()
+    free0, _ = torch.cuda.mem_get_info()
+    for _ in range(3):
+        qcd.norm2_noalloc(x, out)
+    torch.cuda.synchronize()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free1 == free0
+    limit = qcd.noalloc_max_bytes()
+    assert limit == 1 << 30
+    before = out.clone()
+    with pytest.raises(qcd.QcdError) as e:     # the size is checked before anything is enqueued or read
+        qcd.norm2_noalloc(x, out, nreal=limit // 4 + 4)
+    assert e.value.code == qcd.EINVAL and "exceed" in str(e.value)
+    with pytest.raises(qcd.QcdError):
+        qcd.norm2_noalloc(x, out, nreal=6)     # not a whole number of 128-bit words
+    torch.cuda.synchronize()
+    assert torch.equal(out, before)
+    qcd.norm2_noalloc(x, out, nreal=limit // 4 // 1024)   # a size at which the limit check passes still works
+    torch.cuda.synchronize()
+    part = x[: limit // 4 // 1024].double().cpu().numpy()
+    assert abs(out.item() - np.dot(part, part)) <= RTOL * np.dot(part, part)
