@@ -40,8 +40,8 @@
  *                         bit-identical solves, the kernels enqueued past the stopping iteration skip themselves)
  *      QCD_MRHS_TILE=1    multi-right-hand-side hop: opt into the shared-memory tile kernel (slower on B200,
  *                         DESIGN.md section 6); QCD_MRHS_VARIANT=40|41|31|32 picks its staging variant
- *      QCD_PDL=0          launch the hop kernels fully serialised; default: programmatic stream serialisation
- *                         (the next hop launch places its blocks while the previous one drains, and waits on the
+ *      QCD_PDL=0          launch every kernel fully serialised; default: programmatic stream serialisation
+ *                         (the next launch places its blocks while the previous one drains, and waits on the
  *                         device for its completion before it reads anything); same results
  *      QCD_TRACE=1        the mixed solver prints its reliable updates to stderr
  */

@@ -90,6 +90,8 @@ __device__ __forceinline__ bool grid_sum(double v, double* partial, unsigned int
 
 template <typename T> __global__ void __launch_bounds__(BLAS_THREADS) axpby_kernel(DevScalar a, const T* __restrict__ x, DevScalar b, T* __restrict__ y, size_t nvec, const int* halt)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     typedef typename Vec<T>::type V;
     if (halted(halt)) return;
     const T aa = (T)eval(a), bb = (T)eval(b);
@@ -109,6 +111,8 @@ template <typename T> __global__ void __launch_bounds__(BLAS_THREADS) axpby_kern
 template <typename T, int TWO>
 __global__ void __launch_bounds__(BLAS_THREADS) dot_kernel(const T* __restrict__ x, const T* __restrict__ y, size_t nvec, double* partial, unsigned int* ticket, double* out, const int* halt)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     typedef typename Vec<T>::type V;
     if (halted(halt)) return;
     const V* xv = reinterpret_cast<const V*>(x);
@@ -147,6 +151,8 @@ template <typename T>
 __global__ void __launch_bounds__(BLAS_THREADS) cg_update_kernel(DevScalar a, const T* __restrict__ p, const T* __restrict__ q, T* __restrict__ x, T* __restrict__ r, size_t nvec, double* partial,
                                  unsigned int* ticket, double* out, CgCtl* ctl, int* status)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     typedef typename Vec<T>::type V;
     if (ctl) {
         if (halted(&ctl->halt)) return;
@@ -195,6 +201,8 @@ template <typename T>
 __global__ void __launch_bounds__(BLAS_THREADS) cg_xp_kernel(DevScalar a, DevScalar b, const T* __restrict__ r, T* __restrict__ x, T* __restrict__ p, size_t nvec, const CgCtl* ctl,
                              int iter)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     typedef typename Vec<T>::type V;
     const int h = *reinterpret_cast<const volatile int*>(&ctl->halt);
     if (h == CG_BREAKDOWN || (h != CG_RUN && ctl->iter != iter)) return;
@@ -234,6 +242,8 @@ __device__ __forceinline__ size_t hi_index(size_t i, size_t Vh)
 /* y_hi += x_lo ; x_lo = 0   (reliable update, reading O7) */
 __global__ void __launch_bounds__(BLAS_THREADS) accumulate_hi_kernel(double* y, float* x, size_t n4, size_t Vh)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     float4* xv = reinterpret_cast<float4*>(x);
     double2* yv = reinterpret_cast<double2*>(y);
     for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < n4; i += (size_t)gridDim.x * BLAS_THREADS) {
@@ -251,6 +261,8 @@ __global__ void __launch_bounds__(BLAS_THREADS) accumulate_hi_kernel(double* y, 
 __global__ void __launch_bounds__(BLAS_THREADS) residual_hi_kernel(double* rh, float* rl, const double* b, const double* t, size_t n4, size_t Vh,
                                    double* partial, unsigned int* ticket, double* out, CgCtl* ctl)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     double s = 0.0;
     const double2* bv = reinterpret_cast<const double2*>(b);
     const double2* tv = reinterpret_cast<const double2*>(t);
@@ -280,6 +292,8 @@ __global__ void __launch_bounds__(BLAS_THREADS) residual_hi_kernel(double* rh, f
 /* HI_TO_LO: lo = (float) hi ; else hi = (double) lo */
 template <int HI_TO_LO> __global__ void __launch_bounds__(BLAS_THREADS) convert_kernel(double* hi, float* lo, size_t n4, size_t Vh)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     float4* lv = reinterpret_cast<float4*>(lo);
     double2* hv = reinterpret_cast<double2*>(hi);
     for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < n4; i += (size_t)gridDim.x * BLAS_THREADS) {
@@ -300,6 +314,8 @@ template <typename T>
 __global__ void __launch_bounds__(BLAS_THREADS) multishift_x_kernel(MultiShiftCoef cf, T* x, const T* p, size_t fstride_vec, const T* q, T* r,
                                     size_t nvec, double* partial, unsigned int* ticket, double* out)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     typedef typename Vec<T>::type V;
     const V* qv = reinterpret_cast<const V*>(q);
     V* rv = reinterpret_cast<V*>(r);
@@ -335,6 +351,8 @@ __global__ void __launch_bounds__(BLAS_THREADS) multishift_x_kernel(MultiShiftCo
 template <typename T>
 __global__ void __launch_bounds__(BLAS_THREADS) multishift_p_kernel(MultiShiftCoef zeta, MultiShiftCoef beta, T* p, size_t fstride_vec, const T* r, size_t nvec)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     typedef typename Vec<T>::type V;
     const V* rv = reinterpret_cast<const V*>(r);
 #pragma unroll BLAS_UNROLL_N
@@ -376,10 +394,10 @@ int blas_axpby(qcd_ctx* ctx, DevScalar a, const void* x, DevScalar b, void* y, s
 {
     if (prec == 4) {
         const size_t nv = nreal / 4;
-        axpby_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const float*)x, b, (float*)y, nv, halt);
+        launch_pdl(axpby_kernel<float>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, a, (const float*)x, b, (float*)y, nv, halt);
     } else {
         const size_t nv = nreal / 2;
-        axpby_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const double*)x, b, (double*)y, nv, halt);
+        launch_pdl(axpby_kernel<double>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, a, (const double*)x, b, (double*)y, nv, halt);
     }
     return check_launch(ctx, "axpby");
 }
@@ -388,10 +406,10 @@ int blas_norm2(qcd_ctx* ctx, const void* x, size_t nreal, int prec, double* d_ou
 {
     if (prec == 4) {
         const size_t nv = nreal / 4;
-        dot_kernel<float, 0><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const float*)x, (const float*)x, nv, ctx->d_partial, ctx->d_ticket, d_out, nullptr);
+        launch_pdl(dot_kernel<float, 0>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, (const float*)x, (const float*)x, nv, ctx->d_partial, ctx->d_ticket, d_out, nullptr);
     } else {
         const size_t nv = nreal / 2;
-        dot_kernel<double, 0><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const double*)x, (const double*)x, nv, ctx->d_partial, ctx->d_ticket, d_out, nullptr);
+        launch_pdl(dot_kernel<double, 0>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, (const double*)x, (const double*)x, nv, ctx->d_partial, ctx->d_ticket, d_out, nullptr);
     }
     return check_launch(ctx, "norm2");
 }
@@ -400,10 +418,10 @@ int blas_redot(qcd_ctx* ctx, const void* x, const void* y, size_t nreal, int pre
 {
     if (prec == 4) {
         const size_t nv = nreal / 4;
-        dot_kernel<float, 1><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const float*)x, (const float*)y, nv, ctx->d_partial, ctx->d_ticket, d_out, halt);
+        launch_pdl(dot_kernel<float, 1>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, (const float*)x, (const float*)y, nv, ctx->d_partial, ctx->d_ticket, d_out, halt);
     } else {
         const size_t nv = nreal / 2;
-        dot_kernel<double, 1><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>((const double*)x, (const double*)y, nv, ctx->d_partial, ctx->d_ticket, d_out, halt);
+        launch_pdl(dot_kernel<double, 1>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, (const double*)x, (const double*)y, nv, ctx->d_partial, ctx->d_ticket, d_out, halt);
     }
     return check_launch(ctx, "redot");
 }
@@ -413,11 +431,11 @@ int blas_cg_update(qcd_ctx* ctx, DevScalar a, const void* p, const void* q, void
 {
     if (prec == 4) {
         const size_t nv = nreal / 4;
-        cg_update_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const float*)p, (const float*)q, (float*)x, (float*)r, nv,
+        launch_pdl(cg_update_kernel<float>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, a, (const float*)p, (const float*)q, (float*)x, (float*)r, nv,
                                                                                    ctx->d_partial, ctx->d_ticket, d_out, ctl, status);
     } else {
         const size_t nv = nreal / 2;
-        cg_update_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, (const double*)p, (const double*)q, (double*)x, (double*)r, nv,
+        launch_pdl(cg_update_kernel<double>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, a, (const double*)p, (const double*)q, (double*)x, (double*)r, nv,
                                                                                     ctx->d_partial, ctx->d_ticket, d_out, ctl, status);
     }
     return check_launch(ctx, "cg_update");
@@ -427,10 +445,10 @@ int blas_cg_xp(qcd_ctx* ctx, DevScalar a, DevScalar b, const void* r, void* x, v
 {
     if (prec == 4) {
         const size_t nv = nreal / 4;
-        cg_xp_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, b, (const float*)r, (float*)x, (float*)p, nv, ctl, iter);
+        launch_pdl(cg_xp_kernel<float>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, a, b, (const float*)r, (float*)x, (float*)p, nv, ctl, iter);
     } else {
         const size_t nv = nreal / 2;
-        cg_xp_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(a, b, (const double*)r, (double*)x, (double*)p, nv, ctl, iter);
+        launch_pdl(cg_xp_kernel<double>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, a, b, (const double*)r, (double*)x, (double*)p, nv, ctl, iter);
     }
     return check_launch(ctx, "cg_xp");
 }
@@ -438,14 +456,14 @@ int blas_cg_xp(qcd_ctx* ctx, DevScalar a, DevScalar b, const void* r, void* x, v
 int blas_accumulate_hi(qcd_ctx* ctx, void* y_hi, void* x_lo, size_t nreal, size_t Vh)
 {
     const size_t n4 = nreal / 4;
-    accumulate_hi_kernel<<<grid_for(ctx, n4), BLAS_THREADS, 0, ctx->stream>>>((double*)y_hi, (float*)x_lo, n4, Vh);
+    launch_pdl(accumulate_hi_kernel, grid_for(ctx, n4), BLAS_THREADS, ctx->stream, (double*)y_hi, (float*)x_lo, n4, Vh);
     return check_launch(ctx, "accumulate_hi");
 }
 
 int blas_residual_hi(qcd_ctx* ctx, void* r_hi, void* r_lo, const void* b, const void* t, size_t nreal, size_t Vh, double* d_out, CgCtl* ctl)
 {
     const size_t n4 = nreal / 4;
-    residual_hi_kernel<<<grid_for(ctx, n4), BLAS_THREADS, 0, ctx->stream>>>((double*)r_hi, (float*)r_lo, (const double*)b, (const double*)t, n4, Vh,
+    launch_pdl(residual_hi_kernel, grid_for(ctx, n4), BLAS_THREADS, ctx->stream, (double*)r_hi, (float*)r_lo, (const double*)b, (const double*)t, n4, Vh,
                                                                           ctx->d_partial, ctx->d_ticket, d_out, ctl);
     return check_launch(ctx, "residual_hi");
 }
@@ -456,9 +474,9 @@ int blas_convert(qcd_ctx* ctx, void* dst, int pdst, const void* src, int psrc, s
     const size_t n4 = nreal / 4;
     const int g = grid_for(ctx, n4);
     if (pdst == 4)
-        convert_kernel<1><<<g, BLAS_THREADS, 0, ctx->stream>>>((double*)const_cast<void*>(src), (float*)dst, n4, Vh);
+        launch_pdl(convert_kernel<1>, g, BLAS_THREADS, ctx->stream, (double*)const_cast<void*>(src), (float*)dst, n4, Vh);
     else
-        convert_kernel<0><<<g, BLAS_THREADS, 0, ctx->stream>>>((double*)dst, (float*)const_cast<void*>(src), n4, Vh);
+        launch_pdl(convert_kernel<0>, g, BLAS_THREADS, ctx->stream, (double*)dst, (float*)const_cast<void*>(src), n4, Vh);
     return check_launch(ctx, "convert");
 }
 
@@ -481,11 +499,11 @@ int blas_multishift_x(qcd_ctx* ctx, const MultiShiftCoef& cf, void* x, const voi
 {
     if (prec == 4) {
         const size_t nv = nreal / 4;
-        multishift_x_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(cf, (float*)x, (const float*)p, nv, (const float*)q, (float*)r, nv,
+        launch_pdl(multishift_x_kernel<float>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, cf, (float*)x, (const float*)p, nv, (const float*)q, (float*)r, nv,
                                                                                       ctx->d_partial, ctx->d_ticket, d_out);
     } else {
         const size_t nv = nreal / 2;
-        multishift_x_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(cf, (double*)x, (const double*)p, nv, (const double*)q, (double*)r,
+        launch_pdl(multishift_x_kernel<double>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, cf, (double*)x, (const double*)p, nv, (const double*)q, (double*)r,
                                                                                        nv, ctx->d_partial, ctx->d_ticket, d_out);
     }
     return check_launch(ctx, "multishift_x");
@@ -495,10 +513,10 @@ int blas_multishift_p(qcd_ctx* ctx, const MultiShiftCoef& zeta, const MultiShift
 {
     if (prec == 4) {
         const size_t nv = nreal / 4;
-        multishift_p_kernel<float><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(zeta, beta, (float*)p, nv, (const float*)r, nv);
+        launch_pdl(multishift_p_kernel<float>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, zeta, beta, (float*)p, nv, (const float*)r, nv);
     } else {
         const size_t nv = nreal / 2;
-        multishift_p_kernel<double><<<grid_for(ctx, nv), BLAS_THREADS, 0, ctx->stream>>>(zeta, beta, (double*)p, nv, (const double*)r, nv);
+        launch_pdl(multishift_p_kernel<double>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, zeta, beta, (double*)p, nv, (const double*)r, nv);
     }
     return check_launch(ctx, "multishift_p");
 }

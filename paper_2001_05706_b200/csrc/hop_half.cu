@@ -221,6 +221,8 @@ __device__ __forceinline__ void half_store2(unsigned char* block, size_t Vh, int
 template <int DAG, int MODE, int OUT_F32>
 __global__ void __launch_bounds__(64, HOP_MINBLOCKS_HALF) hop_half_kernel(const HalfHopArgs A)
 {
+    pdl_launch_dependents(); /* launched with launch_pdl (qcd_device.cuh) */
+    pdl_wait();
     if (A.halt && *reinterpret_cast<const volatile int*>(A.halt) != 0) return;
     /* a block of 64 threads works on 128 consecutive sites: thread t on base + t and base + 64 + t */
     const int cba = blockIdx.x * 128 + threadIdx.x;
@@ -306,8 +308,8 @@ __global__ void __launch_bounds__(64, HOP_MINBLOCKS_HALF) hop_half_kernel(const 
 template <int DAG, int MODE> cudaError_t launch_mode(const HalfHopArgs& A, int out_f32, cudaStream_t st)
 {
     const int threads = 64, blocks = (A.geo.Vh + 127) / 128;
-    if (out_f32) hop_half_kernel<DAG, MODE, 1><<<blocks, threads, 0, st>>>(A);
-    else hop_half_kernel<DAG, MODE, 0><<<blocks, threads, 0, st>>>(A);
+    if (out_f32) launch_pdl(hop_half_kernel<DAG, MODE, 1>, blocks, threads, st, A);
+    else launch_pdl(hop_half_kernel<DAG, MODE, 0>, blocks, threads, st, A);
     return cudaGetLastError();
 }
 template <int DAG> cudaError_t launch_dag(const HalfHopArgs& A, int mode, int out_f32, cudaStream_t st)
@@ -324,6 +326,8 @@ template <int DAG> cudaError_t launch_dag(const HalfHopArgs& A, int mode, int ou
 /* fp32 internal blocks <-> 16-bit blocks; one thread per (block, cb) */
 template <int TO_HALF> __global__ void half_convert_kernel(unsigned char* half, float* f32, size_t Vh, int nblocks)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= Vh * (size_t)nblocks) return;
     const size_t blk = i / Vh, cb = i - blk * Vh;
@@ -343,6 +347,8 @@ template <int TO_HALF> __global__ void half_convert_kernel(unsigned char* half, 
 __global__ void xpay_q16_kernel(DevScalar as, const float* r, DevScalar bs, int p_is_zero, float* p, unsigned char* ph, size_t Vh, int nblocks,
                                 const int* halt)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     if (halt && *reinterpret_cast<const volatile int*>(halt) != 0) return;
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= Vh * (size_t)nblocks) return;
@@ -390,8 +396,8 @@ int half_convert(qcd_ctx* ctx, void* half, void* f32, size_t Vh, int nblocks, in
 {
     const size_t n = Vh * (size_t)nblocks;
     const int threads = 128, blocks = (int)((n + threads - 1) / threads);
-    if (to_half) half_convert_kernel<1><<<blocks, threads, 0, ctx->stream>>>((unsigned char*)half, (float*)f32, Vh, nblocks);
-    else half_convert_kernel<0><<<blocks, threads, 0, ctx->stream>>>((unsigned char*)half, (float*)f32, Vh, nblocks);
+    if (to_half) launch_pdl(half_convert_kernel<1>, blocks, threads, ctx->stream, (unsigned char*)half, (float*)f32, Vh, nblocks);
+    else launch_pdl(half_convert_kernel<0>, blocks, threads, ctx->stream, (unsigned char*)half, (float*)f32, Vh, nblocks);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "half convert: %s", cudaGetErrorString(e));
     ctx->launches++;
@@ -403,7 +409,7 @@ int half_xpay_store(qcd_ctx* ctx, DevScalar a, const void* r, DevScalar b, int p
 {
     const size_t n = Vh * (size_t)nblocks;
     const int threads = 128, blocks = (int)((n + threads - 1) / threads);
-    xpay_q16_kernel<<<blocks, threads, 0, ctx->stream>>>(a, (const float*)r, b, p_is_zero, (float*)p, (unsigned char*)ph, Vh, nblocks, halt);
+    launch_pdl(xpay_q16_kernel, blocks, threads, ctx->stream, a, (const float*)r, b, p_is_zero, (float*)p, (unsigned char*)ph, Vh, nblocks, halt);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "half xpay: %s", cudaGetErrorString(e));
     ctx->launches++;

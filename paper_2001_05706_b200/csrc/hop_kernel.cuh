@@ -551,6 +551,8 @@ __global__ void __launch_bounds__(128, (sizeof(T) == 4 ? HOP_MRHS_MINBLOCKS_F32 
 {
     typedef typename Vec<T>::type V;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    pdl_launch_dependents();
+    pdl_wait();
     int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= A.geo.Vh) return;
     if (STAGE) cb = mrhs_site(A.geo, A.tblock, cb);
@@ -579,37 +581,21 @@ template <typename T, int RECON> static cudaError_t hop_cheb_launch(const HopArg
     const int threads = 128;
     const int blocks = (A.geo.Vh + threads - 1) / threads;
     if (A.nvec == 1) {
-        hop_cheb_mrhs_kernel<T, RECON, 0><<<blocks, threads, 0, st>>>(A);
+        launch_pdl(hop_cheb_mrhs_kernel<T, RECON, 0>, blocks, threads, st, A);
         return cudaGetLastError();
     }
     const size_t smem = (size_t)8 * SmemLinks<T, RECON>::NCH * 128 * 16;
     /* the attribute is per device and the call is cheap: set it on every launch rather than cache it per process */
     cudaError_t e = cudaFuncSetAttribute(hop_cheb_mrhs_kernel<T, RECON, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    hop_cheb_mrhs_kernel<T, RECON, 1><<<blocks, threads, smem, st>>>(A);
+    launch_pdl_smem(hop_cheb_mrhs_kernel<T, RECON, 1>, blocks, threads, smem, st, A);
     return cudaGetLastError();
-}
-
-/* QCD_PDL=0 in the environment launches the hop kernels fully serialised (A/B switch; default on) */
-static inline bool pdl_enabled()
-{
-    static const int on = [] { const char* e = getenv("QCD_PDL"); return (e && atoi(e) == 0) ? 0 : 1; }();
-    return on != 0;
 }
 
 template <typename T, int RECON, int DAG, int MODE> static cudaError_t hop_launch_pdl(const HopArgs<T>& A, int blocks, int threads, cudaStream_t st)
 {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)blocks);
-    cfg.blockDim = dim3((unsigned)threads);
-    cfg.dynamicSmemBytes = 0;
-    cfg.stream = st;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at;
-    cfg.numAttrs = pdl_enabled() ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, hop_kernel<T, RECON, DAG, MODE>, A);
+    launch_pdl(hop_kernel<T, RECON, DAG, MODE>, blocks, threads, st, A);
+    return cudaGetLastError();
 }
 
 template <typename T, int RECON, int DAG> static cudaError_t hop_dispatch_mode(const HopArgs<T>& A, int mode, cudaStream_t st)

@@ -7,12 +7,44 @@
 #define QCD_DEVICE_CUH
 
 #include "qcd_internal.h"
+#include <cstdlib>
 
 /* programmatic dependent launch (sm_90+): griddepcontrol.launch_dependents lets the next launch of the stream start
  * placing blocks once every block of this grid has executed it; griddepcontrol.wait blocks until the previous grid has
  * completed and its memory operations are visible.  Both are no-ops in a launch without the attribute. */
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+/* QCD_PDL=0 in the environment launches every kernel fully serialised (A/B switch; default on) */
+static inline bool pdl_enabled()
+{
+    static const int on = [] { const char* e = getenv("QCD_PDL"); return (e && atoi(e) == 0) ? 0 : 1; }();
+    return on != 0;
+}
+
+/* Launch with programmatic stream serialisation.  Only for kernels whose first statements are pdl_launch_dependents();
+ * pdl_wait(): such a kernel may be placed while its predecessor in the stream drains and reads or writes nothing
+ * before the predecessor has completed.  The launch error, if any, is left for cudaGetLastError(). */
+template <typename... Exp, typename... Act>
+static inline void launch_pdl_smem(void (*kernel)(Exp...), int grid, int block, size_t smem, cudaStream_t st, Act&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = pdl_enabled() ? 1 : 0;
+    (void)cudaLaunchKernelEx(&cfg, kernel, static_cast<Exp>(args)...);
+}
+template <typename... Exp, typename... Act>
+static inline void launch_pdl(void (*kernel)(Exp...), int grid, int block, cudaStream_t st, Act&&... args)
+{
+    launch_pdl_smem(kernel, grid, block, 0, st, static_cast<Act&&>(args)...);
+}
 
 template <typename T> struct Vec;
 template <> struct Vec<float> {
