@@ -565,3 +565,60 @@ def test_even_odd_helpers_argument_errors():
         c.eo_prepare(blocks(pb)[0], pb)         # bhat inside b
     with pytest.raises(qcd.QcdError):
         c.eo_reconstruct(pb, pb)                # x is b
+
+
+_PDL_SCRIPT = r"""
+import hashlib, sys
+import numpy as np, torch
+from paper_2001_05706_b200 import inputs, qcd
+c = qcd.Context(0)
+dims, kappa, csw = (8, 8, 8, 8), 0.1355, 1.0
+U = inputs.gauge_field(dims, 0.5, 0)
+dU = torch.from_numpy(np.ascontiguousarray(U)).cuda()
+g_hi = c.gauge_load(dU, dims, 8, 18, -1)
+g_lo = c.gauge_load(dU, dims, 4, 12, -1)
+g_q = c.gauge_load(dU, dims, 2, 12, -1)
+c_hi, c_lo, c_q = (c.clover_build(g_hi, kappa, csw, p) for p in (8, 4, 2))
+c.ensure_workspace(c.workspace_bytes(dims, 8))
+b = c.spinor_pack(torch.from_numpy(inputs.spinor_field(dims, 0, 1)).cuda(), dims)
+h = b.numel() // 2
+out = []
+for lo, clo in ((None, None), (g_lo, c_lo), (g_q, c_q)):
+    c.set_operator(g_hi, lo, c_hi, clo, kappa, csw, 0, 0.1)
+    x = torch.zeros_like(b[:h])
+    rc, st = c.cg_solve(x, b[:h].clone(), 1e-10, 5000)
+    out.append(x)
+    print(rc, st.iters, st.reliable_updates)
+v = c.spinor_pack(torch.from_numpy(inputs.round_to_f32(inputs.spinor_field(dims, 1, 0))).float().cuda(), dims)
+vv = torch.cat([v, 2 * v, -v])
+y = torch.empty_like(vv)
+c.cheb_apply_multi(y, vv, 3, g_lo, 0.2, [0.3, -0.2, 0.5, 0.1, -0.4], 2.6)
+out.append(y)
+c.ensure_workspace((4 + 3) * h * 8)
+c.set_operator(g_hi, None, c_hi, None, kappa, csw, 0)
+xs = torch.empty(3 * h, dtype=b.dtype, device="cuda")
+rc, st, rt = c.cg_multishift(xs, b[:h].clone(), [0.0, 0.05, 0.5], 1e-10, 5000)
+out.append(xs)
+torch.cuda.synchronize()
+for t in out:
+    print(hashlib.sha256(t.cpu().numpy().tobytes()).hexdigest())
+"""
+
+
+def test_programmatic_dependent_launch_does_not_change_any_result():
+    """Every kernel is launched with programmatic stream serialisation by default (QCD_PDL, include/qcd.h) and
+    waits on the device for its predecessor before its first read: the solvers (fp64, mixed, 16-bit inside,
+    multi-shift) and the multi-rhs Chebyshev driver must give the same bits with it switched off.  The switch is
+    read once per process, hence the two child processes."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    outs = []
+    for pdl in ("0", "1"):
+        env = dict(os.environ, QCD_PDL=pdl, PYTHONPATH=root + os.pathsep + os.environ.get("PYTHONPATH", ""))
+        r = subprocess.run([sys.executable, "-c", _PDL_SCRIPT], capture_output=True, text=True, env=env, cwd=root, timeout=600)
+        assert r.returncode == 0, r.stderr[-2000:]
+        outs.append(r.stdout)
+    assert outs[0] == outs[1]
+    assert len(outs[0].split()) == 9 + 5
