@@ -371,6 +371,40 @@ __global__ void __launch_bounds__(BLAS_THREADS) multishift_p_kernel(MultiShiftCo
     }
 }
 
+/* x_j += cx_j p_j (j < cx.ns) and p_j = zeta_j r + beta_j p_j (j < zeta.ns <= cx.ns) in one pass: the multi-shift
+ * iteration whose residual update ran in the operator's epilogue (solver.cu) */
+template <typename T>
+__global__ void __launch_bounds__(BLAS_THREADS) multishift_xp_kernel(MultiShiftCoef cx, MultiShiftCoef zeta, MultiShiftCoef beta, T* x, T* p, size_t fstride_vec,
+                                                                     const T* r, size_t nvec)
+{
+    pdl_launch_dependents();
+    pdl_wait();
+    typedef typename Vec<T>::type V;
+    const V* rv = reinterpret_cast<const V*>(r);
+#pragma unroll 2
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
+        T rs[Vec<T>::reals];
+        if (zeta.ns > 0) vec_get(rv[i], rs);
+        for (int j = 0; j < cx.ns; j++) {
+            V* xv = reinterpret_cast<V*>(x) + (size_t)j * fstride_vec;
+            V* pv = reinterpret_cast<V*>(p) + (size_t)j * fstride_vec;
+            T xs[Vec<T>::reals], ps[Vec<T>::reals];
+            vec_get(xv[i], xs);
+            vec_get(pv[i], ps);
+            const T a = (T)cx.c[j];
+#pragma unroll
+            for (int k = 0; k < Vec<T>::reals; k++) xs[k] += a * ps[k];
+            xv[i] = vec_make(xs);
+            if (j < zeta.ns) {
+                const T z = (T)zeta.c[j], b = (T)beta.c[j];
+#pragma unroll
+                for (int k = 0; k < Vec<T>::reals; k++) ps[k] = z * rs[k] + b * ps[k];
+                pv[i] = vec_make(ps);
+            }
+        }
+    }
+}
+
 int grid_for(const qcd_ctx* ctx, size_t nvec)
 {
     size_t b = (nvec + BLAS_THREADS - 1) / BLAS_THREADS;
@@ -492,6 +526,19 @@ int blas_copy(qcd_ctx* ctx, void* dst, const void* src, size_t bytes)
     cudaError_t e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, ctx->stream);
     if (e != cudaSuccess) return qcd_set_error(QCD_ECUDA, "memcpy: %s", cudaGetErrorString(e));
     return QCD_OK;
+}
+
+int blas_multishift_xp(qcd_ctx* ctx, const MultiShiftCoef& cx, const MultiShiftCoef& zeta, const MultiShiftCoef& beta, void* x, void* p, const void* r,
+                       size_t nreal, int prec)
+{
+    if (prec == 4) {
+        const size_t nv = nreal / 4;
+        launch_pdl(multishift_xp_kernel<float>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, cx, zeta, beta, (float*)x, (float*)p, nv, (const float*)r, nv);
+    } else {
+        const size_t nv = nreal / 2;
+        launch_pdl(multishift_xp_kernel<double>, grid_for(ctx, nv), BLAS_THREADS, ctx->stream, cx, zeta, beta, (double*)x, (double*)p, nv, (const double*)r, nv);
+    }
+    return check_launch(ctx, "multishift_xp");
 }
 
 int blas_multishift_x(qcd_ctx* ctx, const MultiShiftCoef& cf, void* x, const void* p, const void* q, void* r, size_t nreal, int prec,

@@ -223,6 +223,8 @@ struct MultiShiftCoef {
     double c[QCD_MAX_SHIFTS];
 };
 /* r -= alpha q ; *d_out = |r|^2 ; x_j += c[j] p_j */
+int blas_multishift_xp(qcd_ctx*, const MultiShiftCoef& cx, const MultiShiftCoef& zeta, const MultiShiftCoef& beta, void* x, void* p, const void* r,
+                       size_t nreal, int prec);
 int blas_multishift_x(qcd_ctx*, const MultiShiftCoef& cf, void* x, const void* p, const void* q, void* r, size_t nreal,
                       int prec, double* d_out);
 /* p_j = zeta.c[j] r + beta.c[j] p_j */

@@ -498,7 +498,47 @@ int qcd_cg_multishift(qcd_ctx* ctx, void* x, const void* b, const double* shifts
     /* a shifted system whose residual |zeta_s| |r| has reached tol |b| is frozen (reading M1): the
      * shifts ascend, so the active systems are always the first nact */
     int k = 0, conv = (bnorm == 0.0), brk = 0, nact = nshift;
-    while (!conv && k < maxiter) {
+    /* Base shift 0: the iteration runs like the plain CG's (cg_iteration): <p,Np> = |t|^2 from the epilogue of the
+     * launch writing t, q = M^dag t never stored, r -= alpha q and rho' = |r|^2 in the epilogue of the launch that
+     * computes it, then ONE pass over the shifted systems (x_s += c_s p_s ; p_s = zeta_s r + beta_s p_s) once the host
+     * has turned <p,Np> and rho' into this iteration's coefficients: one host round trip per iteration instead of
+     * two, 2 + 3 per shift fewer vector streams.  A base shift > 0 needs |p|^2 as well and takes the loop below. */
+    const bool fused = (shifts[0] == 0.0);
+    while (fused && !conv && k < maxiter) {
+        k++;
+        double *d_rho = d + rho_slot(k - 1), *d_rho2 = d + rho_slot(k);
+        const OpExtra ex1 = {nullptr, d + S_PQ, d + S_NTMP, nullptr, nullptr, nullptr, nullptr, nullptr};
+        RC(op_apply_M(ctx, t, p, tmp, o.g, o.c, o.kappa, o.parity, 0, &ex1));
+        const OpExtra ex2 = {nullptr, d_rho2, d + S_NTMP, r, d_rho, d + S_PQ, nullptr, nullptr};
+        RC(op_apply_M(ctx, q, t, tmp, o.g, o.c, o.kappa, o.parity, 1, &ex2));
+        RC(fetch(ctx, 0, 3));
+        const double pq = h[S_PQ];
+        if (!(pq > 0.0)) { brk = 1; break; } /* the launch computing q has written nothing in this case */
+        const double alpha = rho / pq;
+        MultiShiftCoef cx, cz, cb;
+        cx.ns = nact; cx.alpha = alpha;
+        for (int s = 0; s < nact; s++) {
+            const double sh = shifts[s] - shifts[0];
+            zp[s] = z0[s] * zm[s] * alpha_old / (alpha * beta_old * (zm[s] - z0[s]) + zm[s] * alpha_old * (1.0 + sh * alpha));
+            cx.c[s] = alpha * zp[s] / z0[s];
+        }
+        const double rho2 = h[rho_slot(k)];
+        rnorm = sqrt(rho2);
+        conv = (rnorm <= tol * bnorm);
+        if (!conv) while (nact > 1 && fabs(zp[nact - 1]) * rnorm <= tol * bnorm) nact--;
+        const double beta = rho2 / rho;
+        cz.ns = cb.ns = conv ? 0 : nact; cz.alpha = cb.alpha = 0.0;
+        for (int s = 0; s < cz.ns; s++) {
+            const double ratio = zp[s] / z0[s];
+            cz.c[s] = zp[s];
+            cb.c[s] = beta * ratio * ratio;
+            zm[s] = z0[s];
+            z0[s] = zp[s];
+        }
+        RC(blas_multishift_xp(ctx, cx, cz, cb, x, p, r, o.nreal, P));
+        rho = rho2; alpha_old = alpha; beta_old = beta;
+    }
+    while (!fused && !conv && k < maxiter) {
         k++;
         RC(apply_N(o, q, p, t, tmp));
         if (shifts[0] != 0.0) RC(blas_axpby(ctx, host_scalar(shifts[0]), p, host_scalar(1.0), q, o.nreal, P));
