@@ -207,13 +207,15 @@ def test_chebyshev_multi_rhs_matches_oracle(precision, recon, dims):
     assert relerr(y1.cpu().numpy(), y[:n].cpu().numpy()) <= (1e-6 if precision == 4 else 1e-14)
 
 
-@pytest.mark.parametrize("mode,csw,precision", [(2, 0.0, 8), (0, 1.0, 8), (0, 1.0, 4)])
-def test_multishift_cg_matches_oracle(mode, csw, precision):
-    """(N + sigma_i) x_i = b for all shifts with one N apply per iteration."""
+@pytest.mark.parametrize("mode,csw,precision,base0", [(2, 0.0, 8, False), (0, 1.0, 8, True), (0, 1.0, 4, True), (2, 1.0, 8, True),
+                                                     (0, 1.0, 8, False)])
+def test_multishift_cg_matches_oracle(mode, csw, precision, base0):
+    """(N + sigma_i) x_i = b for all shifts with one N apply per iteration; base shift 0 (iteration
+    fused into the operator's epilogues) and > 0 (separate BLAS kernels), full lattice and even-odd."""
     c = ctx()
     dims, kappa = (8, 8, 8, 16), 0.135
     tol = 1e-10 if precision == 8 else 1e-5
-    shifts = [0.0, 0.01, 0.1, 1.0] if mode == 0 else [0.02, 0.3, 3.0]
+    shifts = [0.0, 0.01, 0.1, 1.0] if base0 else [0.02, 0.3, 3.0]
     U, g, cl, A, Ainv = setup_operator(c, dims, kappa, csw, precision, 18)
     if precision == 4 and A is not None:
         A, Ainv = inputs.round_to_f32(A), inputs.round_to_f32(Ainv)
