@@ -614,13 +614,17 @@ def run_ours(args):
     del hsrc
     c.dslash_host_batch(hout, hin, e2e_steps, g, cl, KAPPA, CSW, 0, 0)        # warm-up (creates the copy streams)
     torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    e0.record()
-    c.dslash_host_batch(hout, hin, e2e_steps, g, cl, KAPPA, CSW, 0, 0)
-    e1.record()
-    torch.cuda.synchronize()
-    e2e_ms = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3) / e2e_steps
-    e2e_ms = max_over_ranks(e2e_ms)
+    # the host side of PCIe is shared with whatever else runs on the box: three timed calls of e2e_steps steps
+    # each, the median reported (all three kept in the line)
+    e2e_reps = []
+    for _ in range(3):
+        t0 = time.perf_counter()
+        e0.record()
+        c.dslash_host_batch(hout, hin, e2e_steps, g, cl, KAPPA, CSW, 0, 0)
+        e1.record()
+        torch.cuda.synchronize()
+        e2e_reps.append(max_over_ranks(max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3) / e2e_steps))
+    e2e_ms = sorted(e2e_reps)[1]
     for _ in range(2):
         c.dslash_host(hout[:h], hin[:h], g, cl, KAPPA, CSW, 0, 0)
     torch.cuda.synchronize()
@@ -631,7 +635,8 @@ def run_ours(args):
     sync_ms = max_over_ranks((time.perf_counter() - t0) * 1e3 / e2e_steps)
     e2e = {"value": round(job_value(world, step_flops(Vh), e2e_ms), 1), "unit": UNIT,
            "h2d_bytes_per_step": blk_bytes, "d2h_bytes_per_step": blk_bytes, "ms_per_step": round(e2e_ms, 4),
-           "steps": e2e_steps, "call": "qcd_dslash_host_batch (pipelined H2D / Mhat / D2H, pinned host buffers)",
+           "steps": e2e_steps, "ms_per_step_of_each_timed_call": [round(v, 4) for v in e2e_reps],
+           "call": "qcd_dslash_host_batch (pipelined H2D / Mhat / D2H, pinned host buffers)",
            "one_call_per_step": {"value": round(job_value(world, step_flops(Vh), sync_ms), 1), "ms_per_step": round(sync_ms, 4),
                                  "call": "qcd_dslash_host"}}
     del hin, hout
