@@ -54,6 +54,7 @@ def parse_args():
     ap.add_argument("--no-config4", action="store_true", help="skip the 48^3x96 Chebyshev workload (configs[4])")
     ap.add_argument("--config4-only", action="store_true", help="only the configs[4] section (for ncu passes)")
     ap.add_argument("--cheb-degree", type=int, default=100, help="Chebyshev degree timed in the configs[4] section")
+    ap.add_argument("--cheb-batches", default="1,12", help="vectors per launch timed in the configs[4] section (divisors of 12)")
     ap.add_argument("--table-scale", type=float, default=1.0, help="scale the iteration counts of the kernel table")
     ap.add_argument("--l2-probe", action="store_true", help="only: read rate of qcd_redot on L2-resident vectors (L2 -> SM fabric)")
     return ap.parse_args()
@@ -366,7 +367,13 @@ def solver_table(c, w):
     return out
 
 
-def config_table(c, peak, config4, only4=False, cheb_degree=100):
+def cheb_batches(args):
+    nbs = tuple(int(v) for v in args.cheb_batches.split(","))
+    assert all(nb >= 1 and 12 % nb == 0 for nb in nbs), "--cheb-batches: divisors of 12"
+    return nbs
+
+
+def config_table(c, peak, config4, only4=False, cheb_degree=100, cheb_batches=(1, 12)):
     """The other BASELINE.json configs at their full sizes (parity for each is in tests/)."""
     import torch
     from paper_2001_05706_b200 import inputs
@@ -446,7 +453,7 @@ def config_table(c, peak, config4, only4=False, cheb_degree=100):
         del dU
         coeff = inputs.chebyshev_sign_coefficients(100)[:cheb_degree + 1]
         res = {}
-        for nb in (1, 12):
+        for nb in cheb_batches:
             v = torch.randn(nb * V * 24, device="cuda", dtype=torch.float32)
             y = torch.empty_like(v)
             c.set_workspace(None)
@@ -663,11 +670,11 @@ def run_ours(args):
             line["cg"] = solver_table(c, w)
             del w
             torch.cuda.empty_cache()
-            line["configs"] = config_table(c, peak, not args.no_config4, cheb_degree=args.cheb_degree)
+            line["configs"] = config_table(c, peak, not args.no_config4, cheb_degree=args.cheb_degree, cheb_batches=cheb_batches(args))
     if args.config4_only and rank == 0:
         del w
         torch.cuda.empty_cache()
-        line["configs"] = config_table(c, peak, True, only4=True, cheb_degree=args.cheb_degree)
+        line["configs"] = config_table(c, peak, True, only4=True, cheb_degree=args.cheb_degree, cheb_batches=cheb_batches(args))
     print(json.dumps(line))
     if world > 1:
         dist.barrier()
