@@ -50,12 +50,15 @@ def test_norm2_noalloc_allocates_nothing_and_rejects_what_the_scratch_cannot_cov
     out = torch.zeros(1, dtype=torch.float64, device="cuda")
     qcd.norm2_noalloc(x, out)                  # first launch: the kernel's code is loaded now
     torch.cuda.synchronize()
-    free0, _ = torch.cuda.mem_get_info()
-    for _ in range(3):
-        qcd.norm2_noalloc(x, out)
-    torch.cuda.synchronize()
-    free1, _ = torch.cuda.mem_get_info()
-    assert free1 == free0
+    unchanged = False
+    for _ in range(3):                         # free device memory is global to the GPU: allow for an unrelated change
+        free0, _ = torch.cuda.mem_get_info()
+        for _ in range(3):
+            qcd.norm2_noalloc(x, out)
+        torch.cuda.synchronize()
+        free1, _ = torch.cuda.mem_get_info()
+        unchanged = unchanged or free1 == free0
+    assert unchanged
     limit = qcd.noalloc_max_bytes()
     assert limit == 1 << 30
     before = out.clone()
