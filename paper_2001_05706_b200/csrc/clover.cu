@@ -88,17 +88,39 @@ __device__ inline M3 dag(const M3& a)
     return c;
 }
 
+/* c = a b, a b^dag (DB) */
+template <int DB> __device__ __forceinline__ M3 mulx(const M3& a, const M3& b)
+{
+    M3 c;
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            cplx s = {0, 0};
+#pragma unroll
+            for (int k = 0; k < 3; k++) s = cadd(s, cmul(a.m[3 * i + k], DB ? cconj(b.m[3 * j + k]) : b.m[3 * k + j]));
+            c.m[3 * i + j] = s;
+        }
+    return c;
+}
+
 template <typename T, int RECON> struct LinkReader {
     const T* data;
     size_t gblock;
     DevGeom g;
-    /* U_mu at site c shifted by dm in direction m and dn in direction n (periodic) */
-    __device__ M3 get(int mu, const Coord& c, int m, int dm, int n, int dn) const
+    /* U_mu at site c shifted by dm in direction m and dn in direction n (periodic); the
+     * shifts are -1, 0 or +1 */
+    __device__ __forceinline__ M3 get(int mu, const Coord& c, int m, int dm, int n, int dn) const
     {
         int x[4] = {c.x, c.y, c.z, c.t};
         const int L[4] = {g.X, g.Y, g.Z, g.T};
-        x[m] = (x[m] + dm + L[m]) % L[m];
-        x[n] = (x[n] + dn + L[n]) % L[n];
+#pragma unroll
+        for (int k = 0; k < 4; k++) { /* selects, not indexing: m and n are loop variables of a rolled loop */
+            const int sh = (k == m ? dm : 0) + (k == n ? dn : 0);
+            int v = x[k] + sh;
+            v = v < 0 ? v + L[k] : (v >= L[k] ? v - L[k] : v);
+            x[k] = v;
+        }
         const int parity = (x[0] + x[1] + x[2] + x[3]) & 1;
         const int cb = coord_to_cb(g, x[0], x[1], x[2], x[3]);
         T u[18];
@@ -110,90 +132,113 @@ template <typename T, int RECON> struct LinkReader {
     }
 };
 
-__device__ inline int tri_index(int hi, int lo) { return 5 * lo - (lo * (lo - 1)) / 2 + (hi - lo - 1); }
+__host__ __device__ constexpr int tri_index(int hi, int lo) { return 5 * lo - (lo * (lo - 1)) / 2 + (hi - lo - 1); }
 
-/* in-place inverse of a 6x6 complex matrix, Gauss-Jordan with partial pivoting */
-__device__ bool invert6(cplx (*a)[6])
+/* Packed Hermitian 6x6 block (the storage format): p[0..5] the diagonal, p[6 + 2 t], p[7 + 2 t] = Re, Im of a[hi][lo],
+ * t = tri_index(hi, lo), hi > lo.  In-place inverse through p = L D L^dag (L unit lower triangular, D real), M = L^-1,
+ * p^-1 = M^dag D^-1 M; every index is a compile-time constant, the 36 reals stay in registers.  No pivoting:
+ * A = 1 + kappa csw C is positive definite for every physical (kappa, csw); a vanishing or non-finite pivot
+ * reports the block as singular. */
+__device__ __forceinline__ cplx pk_get(const double (&p)[36], int hi, int lo) { return {p[6 + 2 * tri_index(hi, lo)], p[7 + 2 * tri_index(hi, lo)]}; }
+__device__ __forceinline__ void pk_set(double (&p)[36], int hi, int lo, cplx v)
 {
-    cplx inv[6][6];
-    for (int i = 0; i < 6; i++)
-        for (int j = 0; j < 6; j++) inv[i][j] = {i == j ? 1.0 : 0.0, 0.0};
-    for (int col = 0; col < 6; col++) {
-        int piv = col;
-        double best = a[col][col].re * a[col][col].re + a[col][col].im * a[col][col].im;
-        for (int r = col + 1; r < 6; r++) {
-            const double v = a[r][col].re * a[r][col].re + a[r][col].im * a[r][col].im;
-            if (v > best) { best = v; piv = r; }
+    p[6 + 2 * tri_index(hi, lo)] = v.re;
+    p[7 + 2 * tri_index(hi, lo)] = v.im;
+}
+__device__ __forceinline__ bool invert_packed(double (&p)[36])
+{
+    bool ok = true;
+    /* p = L D L^dag in place: diagonal <- 1 / d_j, lower triangle <- L */
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+        double dj = p[j];
+#pragma unroll
+        for (int k = 0; k < j; k++) {
+            const cplx l = pk_get(p, j, k);
+            dj -= (l.re * l.re + l.im * l.im) / p[k];
         }
-        if (!(best > 0.0)) return false;
-        if (piv != col)
-            for (int j = 0; j < 6; j++) {
-                cplx t = a[col][j]; a[col][j] = a[piv][j]; a[piv][j] = t;
-                t = inv[col][j]; inv[col][j] = inv[piv][j]; inv[piv][j] = t;
+        ok = ok && (fabs(dj) > 1e-300) && (fabs(dj) < 1e300);
+        const double dinv = 1.0 / dj;
+#pragma unroll
+        for (int i = j + 1; i < 6; i++) {
+            cplx v = pk_get(p, i, j);
+#pragma unroll
+            for (int k = 0; k < j; k++) {
+                const cplx t = cmul(pk_get(p, i, k), cconj(pk_get(p, j, k)));
+                v.re -= t.re / p[k];
+                v.im -= t.im / p[k];
             }
-        const cplx p = a[col][col];
-        const double d = p.re * p.re + p.im * p.im;
-        const cplx pinv = {p.re / d, -p.im / d};
-        for (int j = 0; j < 6; j++) {
-            a[col][j] = cmul(a[col][j], pinv);
-            inv[col][j] = cmul(inv[col][j], pinv);
+            pk_set(p, i, j, {v.re * dinv, v.im * dinv});
         }
-        for (int r = 0; r < 6; r++) {
-            if (r == col) continue;
-            const cplx f = a[r][col];
-            for (int j = 0; j < 6; j++) {
-                a[r][j] = csub(a[r][j], cmul(f, a[col][j]));
-                inv[r][j] = csub(inv[r][j], cmul(f, inv[col][j]));
-            }
-        }
+        p[j] = dinv;
     }
-    for (int i = 0; i < 6; i++)
-        for (int j = 0; j < 6; j++) a[i][j] = inv[i][j];
-    return true;
+    /* lower triangle <- M = L^-1, column by column (column j needs L of the columns to its right, still in place) */
+#pragma unroll
+    for (int j = 0; j < 6; j++)
+#pragma unroll
+        for (int i = j + 1; i < 6; i++) {
+            cplx v = pk_get(p, i, j);
+#pragma unroll
+            for (int k = j + 1; k < i; k++) v = cadd(v, cmul(pk_get(p, i, k), pk_get(p, k, j)));
+            pk_set(p, i, j, {-v.re, -v.im});
+        }
+    /* p <- M^dag D^-1 M, row by row from the top: entry (i,j) needs rows >= i only, its own row only at (i,j) itself */
+#pragma unroll
+    for (int i = 0; i < 6; i++) {
+#pragma unroll
+        for (int j = 0; j < i; j++) {
+            const cplx mij = pk_get(p, i, j);
+            cplx s = {mij.re * p[i], mij.im * p[i]};
+#pragma unroll
+            for (int k = i + 1; k < 6; k++) {
+                const cplx t = cmul(cconj(pk_get(p, k, i)), pk_get(p, k, j));
+                s.re += t.re * p[k];
+                s.im += t.im * p[k];
+            }
+            pk_set(p, i, j, s);
+        }
+        double s = p[i];
+#pragma unroll
+        for (int k = i + 1; k < 6; k++) {
+            const cplx m = pk_get(p, k, i);
+            s += (m.re * m.re + m.im * m.im) * p[k];
+        }
+        p[i] = s;
+    }
+    return ok;
 }
 
-template <typename TS> __device__ void store_block(TS* blk, size_t Vh, size_t cb, int b, cplx (*a)[6])
+template <typename TS> __device__ __forceinline__ void store_block(TS* blk, size_t Vh, size_t cb, int b, const double (&p)[36])
 {
     TS r[36];
-    for (int i = 0; i < 6; i++) r[i] = (TS)a[i][i].re;
-    for (int lo = 0; lo < 6; lo++)
-        for (int hi = lo + 1; hi < 6; hi++) {
-            const int k = 6 + 2 * tri_index(hi, lo);
-            /* Hermitian by construction; store the Hermitian part of the pair */
-            r[k] = (TS)(0.5 * (a[hi][lo].re + a[lo][hi].re));
-            r[k + 1] = (TS)(0.5 * (a[hi][lo].im - a[lo][hi].im));
-        }
+#pragma unroll
+    for (int k = 0; k < 36; k++) r[k] = (TS)p[k];
     store_planes<TS, 36>(blk + (size_t)36 * b * Vh, Vh, cb, r);
 }
 
 /* tag type: 16-bit storage (reading H1) */
 struct HalfTag {};
 
-/* pack both chiral blocks of a site (72 reals, fp32) */
-__device__ void pack_site(float (&r)[72], cplx (*a)[6][6])
-{
-    for (int b = 0; b < 2; b++) {
-        for (int i = 0; i < 6; i++) r[36 * b + i] = (float)a[b][i][i].re;
-        for (int lo = 0; lo < 6; lo++)
-            for (int hi = lo + 1; hi < 6; hi++) {
-                const int k = 36 * b + 6 + 2 * tri_index(hi, lo);
-                r[k] = (float)(0.5 * (a[b][hi][lo].re + a[b][lo][hi].re));
-                r[k + 1] = (float)(0.5 * (a[b][hi][lo].im - a[b][lo][hi].im));
-            }
-    }
-}
-__device__ void store_site_half(unsigned char* blk, size_t Vh, size_t cb, cplx (*a)[6][6])
+/* both chiral blocks of a site (72 reals) -> int16 codes + site norm */
+__device__ __forceinline__ void store_site_half(unsigned char* blk, size_t Vh, size_t cb, const double (&p0)[36], const double (&p1)[36])
 {
     float r[72];
-    pack_site(r, a);
+#pragma unroll
+    for (int k = 0; k < 36; k++) { r[k] = (float)p0[k]; r[36 + k] = (float)p1[k]; }
     float n = 0.f;
+#pragma unroll
     for (int k = 0; k < 72; k++) n = fmaxf(n, fabsf(r[k]));
     const float scale = n > 0.f ? __fdiv_rn(32767.0f, n) : 0.f;
     int4* q = reinterpret_cast<int4*>(blk) + cb;
+#pragma unroll
     for (int c = 0; c < 9; c++) q[(size_t)c * Vh] = half_pack8(&r[8 * c], scale);
     reinterpret_cast<float*>(blk + Vh * 144)[cb] = n;
 }
 
+/* One thread per site.  The six planes, the four leaves of each and all matrix indices are unrolled, so the two
+ * packed blocks (72 reals) and the running products live in registers: round 1's kernel kept two dense 6x6 complex
+ * blocks and the Gauss-Jordan work matrix in 1744 B of dynamically indexed local memory per thread, which
+ * fell out of L2 next to the streamed links (ncu: 21 GB of DRAM traffic for 2.4 GB of links and output). */
 template <typename T, int RECON, typename TS>
 __global__ void __launch_bounds__(64) clover_build_kernel(LinkReader<T, RECON> R, TS* A, TS* Ainv, size_t cblock, double coeff, int* bad)
 {
@@ -203,60 +248,68 @@ __global__ void __launch_bounds__(64) clover_build_kernel(LinkReader<T, RECON> R
     const int parity = i / g.Vh, cb = i - parity * g.Vh;
     const Coord c = cb_to_coord(g, cb, parity);
 
-    cplx blk[2][6][6];
+    double P[2][36];
+#pragma unroll
     for (int b = 0; b < 2; b++)
-        for (int r = 0; r < 6; r++)
-            for (int s = 0; s < 6; s++) blk[b][r][s] = {0.0, 0.0};
+#pragma unroll
+        for (int k = 0; k < 36; k++) P[b][k] = 0.0;
 
-    int pl = 0;
-    for (int m = 0; m < 4; m++)
-        for (int n = m + 1; n < 4; n++, pl++) {
+#pragma unroll 1
+    for (int pl = 0; pl < 6; pl++) {
+        {
+            const int m = pl < 3 ? 0 : (pl < 5 ? 1 : 2), n = pl < 3 ? pl + 1 : (pl < 5 ? pl - 1 : 3);
             /* the four leaves, each a closed loop x -> ... -> x, counter-clockwise in (m,n) */
-            M3 q = mul(mul(R.get(m, c, m, 0, n, 0), R.get(n, c, m, 1, n, 0)),
-                       mul(dag(R.get(m, c, m, 0, n, 1)), dag(R.get(n, c, m, 0, n, 0))));
-            M3 l = mul(mul(R.get(n, c, m, 0, n, 0), dag(R.get(m, c, m, -1, n, 1))),
-                       mul(dag(R.get(n, c, m, -1, n, 0)), R.get(m, c, m, -1, n, 0)));
+            M3 q = mulx<1>(mulx<1>(mulx<0>(R.get(m, c, m, 0, n, 0), R.get(n, c, m, 1, n, 0)), R.get(m, c, m, 0, n, 1)), R.get(n, c, m, 0, n, 0));
+            M3 l = mulx<0>(mulx<1>(mulx<1>(R.get(n, c, m, 0, n, 0), R.get(m, c, m, -1, n, 1)), R.get(n, c, m, -1, n, 0)), R.get(m, c, m, -1, n, 0));
+#pragma unroll
             for (int k = 0; k < 9; k++) q.m[k] = cadd(q.m[k], l.m[k]);
-            l = mul(mul(dag(R.get(m, c, m, -1, n, 0)), dag(R.get(n, c, m, -1, n, -1))),
-                    mul(R.get(m, c, m, -1, n, -1), R.get(n, c, m, 0, n, -1)));
+            l = mulx<0>(mulx<0>(mulx<1>(dag(R.get(m, c, m, -1, n, 0)), R.get(n, c, m, -1, n, -1)), R.get(m, c, m, -1, n, -1)), R.get(n, c, m, 0, n, -1));
+#pragma unroll
             for (int k = 0; k < 9; k++) q.m[k] = cadd(q.m[k], l.m[k]);
-            l = mul(mul(dag(R.get(n, c, m, 0, n, -1)), R.get(m, c, m, 0, n, -1)),
-                    mul(R.get(n, c, m, 1, n, -1), dag(R.get(m, c, m, 0, n, 0))));
+            l = mulx<1>(mulx<0>(mulx<0>(dag(R.get(n, c, m, 0, n, -1)), R.get(m, c, m, 0, n, -1)), R.get(n, c, m, 1, n, -1)), R.get(m, c, m, 0, n, 0));
+#pragma unroll
             for (int k = 0; k < 9; k++) q.m[k] = cadd(q.m[k], l.m[k]);
-            /* Fhat = (Q - Q^dag)/8 */
-            M3 f;
-            for (int a = 0; a < 3; a++)
-                for (int bb = 0; bb < 3; bb++) {
-                    const cplx d = csub(q.m[3 * a + bb], cconj(q.m[3 * bb + a]));
-                    f.m[3 * a + bb] = {0.125 * d.re, 0.125 * d.im};
-                }
-            /* C += (i sigma_mn) (x) Fhat, chirality block by block */
+            /* Fhat = (Q - Q^dag)/8;  C += (i sigma_mn) (x) Fhat, chirality block by block, lower triangle only */
+#pragma unroll
             for (int b = 0; b < 2; b++)
+#pragma unroll
                 for (int s = 0; s < 2; s++)
-                    for (int sp = 0; sp < 2; sp++) {
+#pragma unroll
+                    for (int sp = 0; sp <= s; sp++) {
                         const cplx sg = c_isigma[pl][2 * b + s][2 * b + sp];
-                        if (sg.re == 0.0 && sg.im == 0.0) continue;
+#pragma unroll
                         for (int a = 0; a < 3; a++)
-                            for (int bb = 0; bb < 3; bb++)
-                                blk[b][3 * s + a][3 * sp + bb] = cadd(blk[b][3 * s + a][3 * sp + bb], cmul(sg, f.m[3 * a + bb]));
+#pragma unroll
+                            for (int bb = 0; bb < 3; bb++) {
+                                const int row = 3 * s + a, col = 3 * sp + bb;
+                                if (row < col) continue;
+                                const cplx dq = csub(q.m[3 * a + bb], cconj(q.m[3 * bb + a]));
+                                const cplx f = {0.125 * dq.re, 0.125 * dq.im};
+                                const cplx v = cmul(sg, f);
+                                if (row == col) P[b][row] += v.re;
+                                else { P[b][6 + 2 * tri_index(row, col)] += v.re; P[b][7 + 2 * tri_index(row, col)] += v.im; }
+                            }
                     }
         }
-
-    for (int b = 0; b < 2; b++)
-        for (int r = 0; r < 6; r++)
-            for (int s = 0; s < 6; s++) {
-                blk[b][r][s].re *= coeff;
-                blk[b][r][s].im *= coeff;
-                if (r == s) blk[b][r][s].re += 1.0;
-            }
-    constexpr bool HALF = std::is_same<TS, HalfTag>::value;
-    if constexpr (HALF) store_site_half(reinterpret_cast<unsigned char*>(A) + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, blk);
-    for (int b = 0; b < 2; b++) {
-        if constexpr (!HALF) store_block<TS>(A + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, b, blk[b]);
-        if (!invert6(blk[b])) atomicAdd(bad, 1);
-        if constexpr (!HALF) store_block<TS>(Ainv + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, b, blk[b]);
     }
-    if constexpr (HALF) store_site_half(reinterpret_cast<unsigned char*>(Ainv) + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, blk);
+
+#pragma unroll
+    for (int b = 0; b < 2; b++)
+#pragma unroll
+        for (int k = 0; k < 36; k++) P[b][k] = P[b][k] * coeff + (k < 6 ? 1.0 : 0.0);
+    constexpr bool HALF = std::is_same<TS, HalfTag>::value;
+    if constexpr (HALF) store_site_half(reinterpret_cast<unsigned char*>(A) + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, P[0], P[1]);
+    else {
+        store_block<TS>(A + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, 0, P[0]);
+        store_block<TS>(A + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, 1, P[1]);
+    }
+    if (!invert_packed(P[0])) atomicAdd(bad, 1);
+    if (!invert_packed(P[1])) atomicAdd(bad, 1);
+    if constexpr (HALF) store_site_half(reinterpret_cast<unsigned char*>(Ainv) + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, P[0], P[1]);
+    else {
+        store_block<TS>(Ainv + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, 0, P[0]);
+        store_block<TS>(Ainv + (size_t)parity * cblock, (size_t)g.Vh, (size_t)cb, 1, P[1]);
+    }
 }
 
 /* expand packed blocks to dense 12x12 complex per site, boundary site order, fp64 */
