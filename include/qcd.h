@@ -114,7 +114,10 @@ int qcd_gauge_free(qcd_gauge* g);
  * leaves, A(x) = 1 + kappa*csw*sum_{mu<nu} i sigma_munu (x) Fhat_munu(x) as two
  * Hermitian 6x6 chiral blocks (2 x (6 real diag + 15 complex) = 72 reals/site) and
  * A^-1; arithmetic in fp64, stored in `precision`.  storage: DEVICE,
- * qcd_clover_bytes(dims, precision) bytes (A then A^-1). */
+ * qcd_clover_bytes(dims, precision) bytes (A then A^-1).  A^-1 is taken block by block
+ * through A = L D L^dag without pivoting (A is positive definite for physical kappa*csw);
+ * QCD_EBREAKDOWN if a block has a vanishing or non-finite pivot (the fields are then
+ * not to be used). */
 size_t qcd_clover_bytes(const int dims[4], int precision);
 int qcd_clover_build(qcd_ctx* ctx, qcd_clover** c, const qcd_gauge* g, void* storage,
                      double kappa, double csw, int precision);
