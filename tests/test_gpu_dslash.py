@@ -238,3 +238,22 @@ def test_wilson_multi_matches_oracle(dims, nvec, precision):
     from paper_2001_05706_b200 import qcd
     with pytest.raises(qcd.QcdError):
         c.wilson_multi(batch, batch, nvec, g, kappa)          # aliased
+
+
+def test_clover_build_reports_a_block_it_cannot_invert():
+    """A non-finite pivot of the L D L^dag factorisation (here from a NaN link) is QCD_EBREAKDOWN, not a silent
+    NaN field; an ordinary field on the same lattice still builds afterwards."""
+    from paper_2001_05706_b200 import qcd
+    c = ctx()
+    dims = (4, 4, 4, 4)
+    U = inputs.gauge_field(dims, 0.5, 0)
+    bad = U.copy()
+    bad[0, 1, 2, 3, 0, 0, 0, 0] = np.nan
+    g = c.gauge_load(to_dev(bad, 8), dims, 8, 18, -1)
+    with pytest.raises(qcd.QcdError) as e:
+        c.clover_build(g, 0.135, 1.0, 8)
+    assert e.value.code == qcd.EBREAKDOWN
+    g = c.gauge_load(to_dev(U, 8), dims, 8, 18, -1)
+    cl = c.clover_build(g, 0.135, 1.0, 8)
+    A, Ainv = oracle_clover(U, dims, 0.135, 1.0)
+    assert relerr(c.clover_unpack(cl, 1).cpu().numpy(), Ainv) <= 1e-12
