@@ -73,3 +73,32 @@ def test_norm2_noalloc_allocates_nothing_and_rejects_what_the_scratch_cannot_cov
     torch.cuda.synchronize()
     part = x[: limit // 4 // 1024].double().cpu().numpy()
     assert abs(out.item() - np.dot(part, part)) <= RTOL * np.dot(part, part)
+
+
+def test_norm2_noalloc_can_be_captured_in_a_cuda_graph_and_replayed():
+    """What the entry point is for: it runs under stream capture (nothing in it allocates or synchronises) and the
+    replayed graph recomputes from the current contents of x."""
+    qcd.noalloc_setup(0)                       # set-up belongs outside the capture
+    x = field(24 * 100000, 4, 11)
+    out = torch.zeros(1, dtype=torch.float64, device="cuda")
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        qcd.norm2_noalloc(x, out)              # uncaptured call on the same stream: loads the kernel, gives the value
+    s.synchronize()
+    want = out.item()
+    x64 = x.double().cpu().numpy()
+    assert abs(want - np.dot(x64, x64)) <= RTOL * want
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        qcd.norm2_noalloc(x, out)
+    out.zero_()
+    torch.cuda.synchronize()
+    g.replay()
+    torch.cuda.synchronize()
+    assert out.item() == want
+    x.mul_(2.0)                                # exact in binary: the sum of squares scales by exactly 4
+    torch.cuda.synchronize()
+    g.replay()
+    torch.cuda.synchronize()
+    assert out.item() == 4.0 * want
