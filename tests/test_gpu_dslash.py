@@ -257,3 +257,41 @@ def test_clover_build_reports_a_block_it_cannot_invert():
     cl = c.clover_build(g, 0.135, 1.0, 8)
     A, Ainv = oracle_clover(U, dims, 0.135, 1.0)
     assert relerr(c.clover_unpack(cl, 1).cpu().numpy(), Ainv) <= 1e-12
+
+
+def test_even_odd_operator_can_be_captured_in_a_cuda_graph():
+    """SURVEY 8(d) caveat (i): at small sizes the launches are what costs; the operator (launched with programmatic
+    stream serialisation) captures into a CUDA graph on the ctx's stream and the replay gives the eager bits."""
+    from paper_2001_05706_b200 import qcd
+    dims, kappa, csw = (8, 8, 8, 16), 0.135, 1.0
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        c = qcd.Context(0, stream=s)
+        U = inputs.round_to_f32(inputs.gauge_field(dims, 0.5, 0))
+        g = c.gauge_load(to_dev(U, 4), dims, 4, 12, -1)
+        cl = c.clover_build(g, kappa, csw, 4)
+        pin = c.spinor_pack(to_dev(inputs.round_to_f32(inputs.spinor_field(dims, 0, 0)), 4), dims)
+        h = pin.numel() // 2
+        src, mid, dst, tmp = pin[:h].clone(), torch.empty_like(pin[:h]), torch.empty_like(pin[:h]), torch.empty_like(pin[:h])
+        c.dslash_ex(mid, src, g, cl, kappa, csw, 0, 0, tmp)
+        c.dslash_ex(dst, mid, g, cl, kappa, csw, 0, qcd.DAGGER, tmp)      # dst = Mhat^dag Mhat src, eagerly
+    s.synchronize()
+    want = dst.clone()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=s):
+        c.dslash_ex(mid, src, g, cl, kappa, csw, 0, 0, tmp)
+        c.dslash_ex(dst, mid, g, cl, kappa, csw, 0, qcd.DAGGER, tmp)
+    dst.zero_()
+    mid.zero_()
+    torch.cuda.synchronize()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(dst, want)
+    src.mul_(2.0)
+    torch.cuda.synchronize()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(dst, 2.0 * want)
+    del graph
+    c.close()
