@@ -298,6 +298,39 @@ int cg_mixed(qcd_ctx* ctx, void* y, const void* b, double tol, int maxiter, qcd_
     return conv ? QCD_OK : QCD_NOCONV;
 }
 
+/* The scalar side of the multi-shift CG (B. Jegerlehner, hep-lat/9612014): zeta_s of the previous, current and next
+ * iteration for every shift, relative to the base shift. */
+struct ShiftRecurrence {
+    double zm[QCD_MAX_SHIFTS], z0[QCD_MAX_SHIFTS], zp[QCD_MAX_SHIFTS];
+    double alpha_old, beta_old;
+    const double* shifts;
+    /* x_s += c_s p_s, c_s = alpha zeta_s' / zeta_s, for the first nact shifts */
+    MultiShiftCoef x_coef(double alpha, int nact)
+    {
+        MultiShiftCoef cx;
+        cx.ns = nact; cx.alpha = alpha;
+        for (int s = 0; s < nact; s++) {
+            const double sh = shifts[s] - shifts[0];
+            zp[s] = z0[s] * zm[s] * alpha_old / (alpha * beta_old * (zm[s] - z0[s]) + zm[s] * alpha_old * (1.0 + sh * alpha));
+            cx.c[s] = alpha * zp[s] / z0[s];
+        }
+        return cx;
+    }
+    /* p_s = zeta_s' r + beta_s p_s, beta_s = beta (zeta_s' / zeta_s)^2; advances the recurrence */
+    void p_coef(double alpha, double beta, int nact, MultiShiftCoef* cz, MultiShiftCoef* cb)
+    {
+        cz->ns = cb->ns = nact; cz->alpha = cb->alpha = 0.0;
+        for (int s = 0; s < nact; s++) {
+            const double ratio = zp[s] / z0[s];
+            cz->c[s] = zp[s];
+            cb->c[s] = beta * ratio * ratio;
+            zm[s] = z0[s];
+            z0[s] = zp[s];
+        }
+        alpha_old = alpha; beta_old = beta;
+    }
+};
+
 double hop_flops_per_apply_M(const Op& o)
 {
     /* nominal (reading S18): 1320 per output site per hop, +504 per clover / clover-inverse apply */
@@ -492,9 +525,10 @@ int qcd_cg_multishift(qcd_ctx* ctx, void* x, const void* b, const double* shifts
     RC(blas_norm2(ctx, b, o.nreal, P, d + S_RHO));
     RC(fetch(ctx, S_RHO, 1));
     const double bnorm = sqrt(h[S_RHO]);
-    double rho = h[S_RHO], alpha_old = 1.0, beta_old = 0.0, rnorm = bnorm;
-    double zm[QCD_MAX_SHIFTS], z0[QCD_MAX_SHIFTS], zp[QCD_MAX_SHIFTS];
-    for (int s = 0; s < nshift; s++) zm[s] = z0[s] = 1.0;
+    double rho = h[S_RHO], rnorm = bnorm;
+    ShiftRecurrence rec;
+    rec.alpha_old = 1.0; rec.beta_old = 0.0; rec.shifts = shifts;
+    for (int s = 0; s < nshift; s++) rec.zm[s] = rec.z0[s] = 1.0;
     /* a shifted system whose residual |zeta_s| |r| has reached tol |b| is frozen (reading M1): the
      * shifts ascend, so the active systems are always the first nact */
     int k = 0, conv = (bnorm == 0.0), brk = 0, nact = nshift;
@@ -515,28 +549,15 @@ int qcd_cg_multishift(qcd_ctx* ctx, void* x, const void* b, const double* shifts
         const double pq = h[S_PQ];
         if (!(pq > 0.0)) { brk = 1; break; } /* the launch computing q has written nothing in this case */
         const double alpha = rho / pq;
-        MultiShiftCoef cx, cz, cb;
-        cx.ns = nact; cx.alpha = alpha;
-        for (int s = 0; s < nact; s++) {
-            const double sh = shifts[s] - shifts[0];
-            zp[s] = z0[s] * zm[s] * alpha_old / (alpha * beta_old * (zm[s] - z0[s]) + zm[s] * alpha_old * (1.0 + sh * alpha));
-            cx.c[s] = alpha * zp[s] / z0[s];
-        }
+        const MultiShiftCoef cx = rec.x_coef(alpha, nact);
         const double rho2 = h[rho_slot(k)];
         rnorm = sqrt(rho2);
         conv = (rnorm <= tol * bnorm);
-        if (!conv) while (nact > 1 && fabs(zp[nact - 1]) * rnorm <= tol * bnorm) nact--;
-        const double beta = rho2 / rho;
-        cz.ns = cb.ns = conv ? 0 : nact; cz.alpha = cb.alpha = 0.0;
-        for (int s = 0; s < cz.ns; s++) {
-            const double ratio = zp[s] / z0[s];
-            cz.c[s] = zp[s];
-            cb.c[s] = beta * ratio * ratio;
-            zm[s] = z0[s];
-            z0[s] = zp[s];
-        }
+        if (!conv) while (nact > 1 && fabs(rec.zp[nact - 1]) * rnorm <= tol * bnorm) nact--;
+        MultiShiftCoef cz, cb;
+        rec.p_coef(alpha, rho2 / rho, conv ? 0 : nact, &cz, &cb); /* the converging iteration updates x only */
         RC(blas_multishift_xp(ctx, cx, cz, cb, x, p, r, o.nreal, P));
-        rho = rho2; alpha_old = alpha; beta_old = beta;
+        rho = rho2;
     }
     while (!fused && !conv && k < maxiter) {
         k++;
@@ -547,31 +568,17 @@ int qcd_cg_multishift(qcd_ctx* ctx, void* x, const void* b, const double* shifts
         const double pq = h[S_PQ];
         if (!(pq > 0.0)) { brk = 1; break; }
         const double alpha = rho / pq;
-        MultiShiftCoef cx;
-        cx.ns = nact; cx.alpha = alpha;
-        for (int s = 0; s < nact; s++) {
-            const double sh = shifts[s] - shifts[0];
-            zp[s] = z0[s] * zm[s] * alpha_old / (alpha * beta_old * (zm[s] - z0[s]) + zm[s] * alpha_old * (1.0 + sh * alpha));
-            cx.c[s] = alpha * zp[s] / z0[s];
-        }
+        const MultiShiftCoef cx = rec.x_coef(alpha, nact);
         RC(blas_multishift_x(ctx, cx, x, p, q, r, o.nreal, P, d + (S_RHO + 1)));
         RC(fetch(ctx, (S_RHO + 1), 1));
         const double rho2 = h[(S_RHO + 1)];
         rnorm = sqrt(rho2);
         if (rnorm <= tol * bnorm) { conv = 1; break; }
-        while (nact > 1 && fabs(zp[nact - 1]) * rnorm <= tol * bnorm) nact--;
-        const double beta = rho2 / rho;
+        while (nact > 1 && fabs(rec.zp[nact - 1]) * rnorm <= tol * bnorm) nact--;
         MultiShiftCoef cz, cb;
-        cz.ns = cb.ns = nact; cz.alpha = cb.alpha = 0.0;
-        for (int s = 0; s < nact; s++) {
-            const double ratio = zp[s] / z0[s];
-            cz.c[s] = zp[s];
-            cb.c[s] = beta * ratio * ratio;
-            zm[s] = z0[s];
-            z0[s] = zp[s];
-        }
+        rec.p_coef(alpha, rho2 / rho, nact, &cz, &cb);
         RC(blas_multishift_p(ctx, cz, cb, p, r, o.nreal, P));
-        rho = rho2; alpha_old = alpha; beta_old = beta;
+        rho = rho2;
     }
     cudaEventRecord(e1, ctx->stream);
     cudaEventSynchronize(e1);
