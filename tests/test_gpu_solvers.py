@@ -624,3 +624,36 @@ def test_programmatic_dependent_launch_does_not_change_any_result():
         outs.append(r.stdout)
     assert outs[0] == outs[1]
     assert len(outs[0].split()) == 9 + 5
+
+
+def test_repeated_solves_give_the_same_bits():
+    """Every reduction is deterministic and every launch waits for its predecessor before its first read
+    (programmatic dependent launch): forty repeats of each solver on a lattice small enough for all blocks of
+    consecutive launches to be resident together give one result."""
+    c = ctx()
+    dims, kappa, csw = (8, 8, 8, 8), 0.1355, 1.0
+    U, g_hi, c_hi, A, Ainv = setup_operator(c, dims, kappa, csw, 8, 18)
+    dU = to_dev(U, 8)
+    g_lo, g_q = c.gauge_load(dU, dims, 4, 12, -1), c.gauge_load(dU, dims, 2, 12, -1)
+    c_lo, c_q = c.clover_build(g_hi, kappa, csw, 4), c.clover_build(g_hi, kappa, csw, 2)
+    pb = pack(c, inputs.spinor_field(dims, 0, 1), dims, 8)
+    src = blocks(pb)[0].clone()
+    h = src.numel()
+    c.ensure_workspace(max(c.workspace_bytes(dims, 8), 7 * h * 8))
+    seen = {}
+    for _ in range(40):
+        for name, lo, clo in (("fp64", None, None), ("mixed", g_lo, c_lo), ("q16", g_q, c_q)):
+            c.set_operator(g_hi, lo, c_hi, clo, kappa, csw, 0, 0.1)
+            x = torch.zeros_like(src)
+            rc, st = c.cg_solve(x, src.clone(), 1e-10, 5000)
+            assert rc == 0
+            seen.setdefault(name, []).append((st.iters, st.reliable_updates, x))
+        c.set_operator(g_hi, None, c_hi, None, kappa, csw, 0)
+        xs = torch.empty(3 * h, dtype=src.dtype, device="cuda")
+        rc, st, _ = c.cg_multishift(xs, src.clone(), [0.0, 0.05, 0.5], 1e-10, 5000)
+        assert rc == 0
+        seen.setdefault("multishift", []).append((st.iters, 0, xs))
+    for name, runs in seen.items():
+        for it, nup, x in runs[1:]:
+            assert (it, nup) == runs[0][:2], name
+            assert torch.equal(x, runs[0][2]), name
